@@ -1,0 +1,157 @@
+/* pbs4d.h -- C-ABI boundary of the B200-native 4D proton dose hot path (arxiv 1809.03927, Pepin et al.).
+ *
+ * The calls follow the paper's statement of the problem (inputs are N_g CT series, N_g-1 deformation
+ * fields and one plan; PAPER.md:53-55 delivery options; PAPER.md:122 accumulation method and subdivision n; output
+ * is one dose on the reference phase) and the names fixed by BASELINE.json north_star:
+ *   set_ct_phases, set_plan_spots, simulate_delivery -> per-phase spot/proton lists, mc_dose_phase,
+ *   accumulate_subvoxel -> 4D dose.
+ *
+ * Conventions.  Grids are C-order [z][y][x] (x fastest); o = corner of voxel (0,0,0), voxel centre = o + (i+1/2) h.
+ * Lengths mm, energies MeV, densities g/cm3, dose Gy.  Pointers named *_dev are DEVICE pointers on the context's
+ * device; everything else is a HOST pointer.  The caller owns every buffer it passes; it must stay valid until the
+ * call returns.  All calls enqueue on the context's stream and synchronise it before returning.
+ * Every function returns PBS4D_OK (0) or a negative error code; nothing throws across the boundary; the message of
+ * the last error is available from pbs4d_last_error().  There is NO CPU fallback: without a CUDA device
+ * pbs4d_create fails with PBS4D_ERR_CUDA.
+ */
+#ifndef PBS4D_H
+#define PBS4D_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PBS4D_OK             0
+#define PBS4D_ERR_ARG       (-1)   /* bad argument                         */
+#define PBS4D_ERR_ORDER     (-2)   /* call-order violation                 */
+#define PBS4D_ERR_CUDA      (-3)   /* CUDA runtime error / no device       */
+#define PBS4D_ERR_NOMEM     (-4)   /* out of host or device memory         */
+#define PBS4D_ERR_OVERFLOW  (-5)   /* fixed-point overflow guard tripped   */
+
+typedef struct pbs4d_ctx pbs4d_ctx;      /* opaque; owns all internal host/device memory */
+
+typedef struct { int32_t nx, ny, nz; float hx, hy, hz, ox, oy, oz; } pbs4d_grid;
+
+/* A treatment field: parallel beam along dir; (eu, ev) span the beam's-eye-view plane through ref.
+ * start_phase = breathing phase in which delivery of this field commences. */
+typedef struct { float dir[3], eu[3], ev[3], ref[3]; int32_t start_phase; } pbs4d_field;
+
+/* A spot = (x, y) position, energy, weight; all spots of one energy form a layer. */
+typedef struct { int32_t field, layer; float x_mm, y_mm, energy_mev, sigma_mm, weight; } pbs4d_spot;
+
+/* Delivery timing model (App. A; values as BASELINE.json configs 3, 5). */
+typedef struct {
+    int32_t  n_phases;             /* N_g breathing phases                                          */
+    int64_t  period_ns;            /* breathing period; phase length = period_ns / n_phases         */
+    int64_t  protons_per_weight;   /* protons of a spot = llround(weight * protons_per_weight)      */
+    int64_t  protons_per_s;        /* spill rate ("spot-spill time")                  */
+    int32_t  ns_per_um;            /* scan speed ("spot-switch time"); 10 m/s -> 100                */
+    int64_t  layer_switch_ns;      /* "layer-switch time"                            */
+    int32_t  repaints;             /* N x layer repainting (BASELINE.json config 5); >= 1           */
+    uint32_t gate_mask;            /* bit p set = beam allowed in phase p (gating)     */
+} pbs4d_delivery_params;
+
+/* One entry of the sub-plans after history allocation. */
+typedef struct {
+    int32_t field, phase, spot, pad;
+    int64_t protons;               /* protons of this spot delivered in this phase by this field    */
+    int64_t first_history;         /* global history index (Philox counter) of its first history    */
+    int64_t n_hist;                /* histories simulated for it (0: dropped)                       */
+    double  weight;                /* protons / n_hist                                              */
+} pbs4d_segment;
+
+/* Result of simulate_delivery; arrays are owned by the context, valid until the next simulate_delivery/destroy.
+ * Segments are sorted by (field, phase, spot). */
+typedef struct {
+    int64_t n_segments; const pbs4d_segment* segments;
+    int32_t n_fields;   const int64_t* field_time_ns;   /* end-of-delivery time per field */
+    int64_t dropped_protons;                            /* protons of segments that got 0 histories */
+    int32_t fixed_shift;                                /* k: dose quantum = 2^-k MeV */
+} pbs4d_phase_lists;
+
+#define PBS4D_NO_MCS       1u      /* test switches: disable Highland deflection / Bohr straggling /       */
+#define PBS4D_NO_STRAGGLE  2u      /* source energy spread / spot size                                      */
+#define PBS4D_NO_ESPREAD   4u
+#define PBS4D_NO_SPOTSIZE  8u
+
+typedef struct {
+    uint64_t histories, steps;
+    int64_t  q_incident, q_deposited, q_escaped;        /* fixed point, quantum 2^-fixed_shift MeV */
+    int32_t  fixed_shift; int32_t pad;
+    float    kernel_ms;                                 /* device time of the transport kernel (CUDA events) */
+} pbs4d_mc_stats;
+
+typedef struct {
+    uint64_t subvoxels, dropped_outside_ref, dropped_outside_dvf;
+    float    push_ms, finalize_ms;                      /* device times (CUDA events) */
+} pbs4d_acc_stats;
+
+/* Create a context on CUDA device `device`; cuda_stream is a cudaStream_t (e.g. torch's current stream) or NULL. */
+int  pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream);
+void pbs4d_destroy(pbs4d_ctx* ctx);
+const char* pbs4d_last_error(const pbs4d_ctx* ctx);
+
+/* a1 (the MC converts Hounsfield units to material density).  hu_dev[p] -> int16 [z][y][x] on grid ct.
+ * Density = piecewise-linear table (hu_pts ascending, n_pts >= 2, clamped at the ends), resampled by overlap-volume
+ * weighted mean onto dose_grid (NULL: dose grid == ct grid).  The context keeps fp32 densities. */
+int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_dev,
+                        const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts);
+
+/* Alternative to set_ct_phases: densities given directly on the dose grid (rho_dev[p] -> fp32 [z][y][x]); copied. */
+int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* dose_grid,
+                             const float* const* rho_dev);
+
+/* Deformation vector field T^{S->R} (Eq. 1; App. B) as displacements [3][z][y][x] (x,y,z components,
+ * mm) at the centres of an axis-aligned grid in the SOURCE phase frame; trilinear in between.
+ * Copied into the context.  Requires set_ct_phases/set_density_phases first. */
+int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
+                  const float* disp_dev);
+
+/* Fields and spots in delivery order (copied). */
+int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fields,
+                         int64_t n_spots, const pbs4d_spot* spots);
+
+/* Optional physics switches for tests (default 0 = full model). */
+int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags);
+
+/* a3: beam-delivery simulation on the host in int64 arithmetic; splits every spot's protons over
+ * the phases it is delivered in and allocates total_histories over the resulting segments. */
+int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
+                            pbs4d_phase_lists* out);
+
+/* a4-a7: Monte Carlo transport of all segments of `phase` on that phase's density grid.
+ * dose_dev (optional) receives fp32 Gy [z][y][x] on the dose grid for the delivered protons (divided by
+ * per_protons if > 0, e.g. "Gy per proton"); rho_dev (optional) receives the density grid (dose and
+ * density are the MC's outputs).  The context keeps the phase dose for accumulate_subvoxel. */
+int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
+                        float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats);
+
+/* Fixed-point energy grid of the last mc_dose_phase call for `phase`, copied to q_dev (int64 [z][y][x]). */
+int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev);
+
+/* a8-a9 (Eq. 2, 4-6): energy-/mass-transfer accumulation with nsx*nsy*nsz subvoxels per voxel of
+ * every source phase that has a DVF to ref_phase, onto ref_phase; masked to the volume covered by all DVFs.
+ * phase_dose_dev: [n_phases] device pointers to fp32 doses on the dose grid, or NULL to use the doses kept by
+ * mc_dose_phase.  dose4d_dev: fp32 [z][y][x] out. */
+int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                              const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats);
+
+/* Integer energy/mass sums of the last accumulate_subvoxel for one source phase (int64 [z][y][x] each). */
+int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev);
+
+/* Whole path with HOST buffers (copies inside): set_ct_phases + set_dvf + set_plan_spots + simulate_delivery +
+ * mc_dose_phase for every phase with protons + accumulate_subvoxel.  hu_host[p], disp_host[p] (NULL = no DVF for p),
+ * dose4d_host out.  seconds (optional, [4]): h2d, delivery, transport, accumulate+d2h wall times. */
+int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_host,
+                        const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts,
+                        const pbs4d_grid* dvf_grid, const float* const* disp_host, int32_t ref_phase,
+                        int32_t n_fields, const pbs4d_field* fields, int64_t n_spots, const pbs4d_spot* spots,
+                        const pbs4d_delivery_params* prm, uint64_t total_histories, uint64_t seed,
+                        int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
+                        double* seconds);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,147 @@
+// Host beam-delivery timeline simulator (Sec. 2.B, App. A).
+//
+// Tracks plan-delivery time against breathing time and splits every spot's protons over the breathing phases they
+// are delivered in -> N_g sub-plans per field.  The paper ran this as a GPU kernel over fields
+// (PAPER.md:51); here it is a few thousand integer events per field, so it runs on the host (BASELINE.json
+// north_star: "a host delivery-timeline simulator").  All arithmetic is int64/int128: the result is unique.
+//
+// Model (BASELINE.json configs 3, 5): spill at protons_per_s, Euclidean scan move at ns_per_um, constant
+// layer-switch time, fixed breathing period, N x layer repainting, gate bitmask.
+#include "internal.h"
+
+#include <algorithm>
+#include <cmath>
+
+namespace pbs4d {
+
+namespace {
+
+using u128 = unsigned __int128;
+constexpr int64_t kNsPerS = 1000000000;
+
+// floor(sqrt(v)) by Newton iteration on integers
+int64_t floor_sqrt(u128 v)
+{
+    if (v == 0) return 0;
+    u128 x = (u128)std::sqrt((double)v) + 2;           // start at or above the root
+    for (;;) {
+        u128 y = (x + v / x) >> 1;
+        if (y >= x) break;
+        x = y;
+    }
+    while (x * x > v) --x;
+    return (int64_t)x;
+}
+
+// Breathing clock of one field: phase bins of length t_ph counted from the start of start_phase.
+struct BreathingClock {
+    int64_t t_ph; int32_t n_phases, start_phase; uint32_t gate;
+    int64_t bin(int64_t t) const { return t / t_ph; }
+    int32_t phase(int64_t t) const { return (int32_t)((bin(t) + start_phase) % n_phases); }
+    int64_t next_edge(int64_t t) const { return (bin(t) + 1) * t_ph; }
+    bool beam_allowed(int64_t t) const { return (gate >> phase(t)) & 1u; }
+};
+
+}  // namespace
+
+int simulate_delivery_host(const std::vector<pbs4d_field>& fields, const std::vector<pbs4d_spot>& spots,
+                           const pbs4d_delivery_params& prm, uint64_t total_histories,
+                           std::vector<pbs4d_segment>& segments, std::vector<int64_t>& field_time_ns,
+                           int64_t& dropped_protons, std::string& err)
+{
+    const int32_t P = prm.n_phases;
+    if (P <= 0 || P > 32) { err = "n_phases must be in [1, 32]"; return PBS4D_ERR_ARG; }
+    if (prm.period_ns < P || prm.protons_per_s <= 0 || prm.repaints <= 0 || prm.ns_per_um < 0 ||
+        prm.layer_switch_ns < 0 || prm.protons_per_weight < 0) { err = "bad delivery parameter"; return PBS4D_ERR_ARG; }
+    const uint32_t all = P == 32 ? 0xFFFFFFFFu : ((1u << P) - 1u);
+    if ((prm.gate_mask & all) == 0) { err = "gate_mask allows no phase"; return PBS4D_ERR_ARG; }
+
+    const size_t nf = fields.size(), ns = spots.size();
+    std::vector<int64_t> delivered(nf * (size_t)P * std::max<size_t>(ns, 1), 0);   // [field][phase][spot]
+    field_time_ns.assign(nf, 0);
+
+    for (size_t f = 0; f < nf; ++f) {
+        BreathingClock clk{ prm.period_ns / P, P, fields[f].start_phase % P, prm.gate_mask };
+        if (clk.start_phase < 0) clk.start_phase += P;
+        int64_t t = 0;
+        bool any_layer = false;
+        size_t i = 0;
+        while (i < ns) {
+            if (spots[i].field != (int32_t)f) { ++i; continue; }
+            size_t end = i;                                     // layer = run of equal layer ids in array order
+            while (end < ns && spots[end].field == (int32_t)f && spots[end].layer == spots[i].layer) ++end;
+            if (any_layer) t += prm.layer_switch_ns;
+            any_layer = true;
+
+            bool beam_positioned = false; int64_t bx = 0, by = 0;
+            for (int32_t paint = 0; paint < prm.repaints; ++paint) {
+                for (size_t s = i; s < end; ++s) {
+                    const int64_t n_spot  = std::llround((double)spots[s].weight * (double)prm.protons_per_weight);
+                    int64_t todo = n_spot / prm.repaints + ((n_spot % prm.repaints) > paint ? 1 : 0);
+                    if (todo <= 0) continue;
+                    const int64_t x_um = std::llround((double)spots[s].x_mm * 1000.0);
+                    const int64_t y_um = std::llround((double)spots[s].y_mm * 1000.0);
+                    if (beam_positioned) {
+                        const u128 ddx = (u128)(x_um > bx ? x_um - bx : bx - x_um);
+                        const u128 ddy = (u128)(y_um > by ? y_um - by : by - y_um);
+                        t += floor_sqrt((ddx * ddx + ddy * ddy) * (u128)prm.ns_per_um * (u128)prm.ns_per_um);
+                    }
+                    beam_positioned = true; bx = x_um; by = y_um;
+
+                    // spill: proton j after the spill clock (re)started at t leaves at t + floor(j * 1e9 / rate)
+                    while (todo > 0) {
+                        if (!clk.beam_allowed(t)) { t = clk.next_edge(t); continue; }      // gate closed: hold
+                        const int64_t window = clk.next_edge(t) - t;                         // ns left in this phase
+                        // protons leaving strictly before the edge: j * 1e9 / rate < window
+                        const u128 cap = ((u128)window * (u128)prm.protons_per_s + (kNsPerS - 1)) / kNsPerS;
+                        const int64_t n = cap < (u128)todo ? (int64_t)cap : todo;
+                        delivered[(f * P + clk.phase(t)) * ns + s] += n;
+                        todo -= n;
+                        t += (int64_t)(((u128)n * kNsPerS) / (u128)prm.protons_per_s);
+                    }
+                }
+            }
+            i = end;
+        }
+        field_time_ns[f] = t;
+    }
+
+    // sub-plans in (field, phase, spot) order, then histories by cumulative rounding
+    segments.clear();
+    u128 total = 0;
+    for (size_t f = 0; f < nf; ++f)
+        for (int32_t p = 0; p < P; ++p)
+            for (size_t s = 0; s < ns; ++s) {
+                const int64_t c = delivered[(f * P + p) * ns + s];
+                if (c <= 0) continue;
+                pbs4d_segment sg{};
+                sg.field = (int32_t)f; sg.phase = p; sg.spot = (int32_t)s; sg.protons = c;
+                segments.push_back(sg);
+                total += (u128)c;
+            }
+    dropped_protons = 0;
+    u128 running = 0; int64_t edge_prev = 0;
+    for (auto& sg : segments) {
+        running += (u128)sg.protons;
+        const int64_t edge = total_histories ? (int64_t)(((u128)total_histories * running) / total) : 0;
+        sg.first_history = edge_prev;
+        sg.n_hist = edge - edge_prev;
+        sg.weight = sg.n_hist > 0 ? (double)sg.protons / (double)sg.n_hist : 0.0;
+        if (total_histories && sg.n_hist == 0) dropped_protons += sg.protons;
+        edge_prev = edge;
+    }
+    return PBS4D_OK;
+}
+
+// Fixed-point shift k: the whole plan's energy (x 1.1) must fit 2^62 quanta even in one voxel.
+int32_t fixed_shift_for(const std::vector<pbs4d_segment>& segments, const std::vector<pbs4d_spot>& spots)
+{
+    double tot = 0.0;
+    for (const auto& sg : segments) tot += (double)sg.protons * (double)spots[sg.spot].energy_mev;
+    tot *= 1.1;
+    if (!(tot > 0.0)) return 40;
+    int32_t k = (int32_t)std::floor(std::log2(4611686018427387904.0 / tot));
+    return std::min(k, 40);
+}
+
+}  // namespace pbs4d

@@ -1,0 +1,113 @@
+// Per-voxel grid kernels: HU -> density ("converting Hounsfield Units to material
+// density") with optional overlap-volume resampling onto the dose grid, and int64 energy -> fp32 dose in Gy.
+// Memory-bound, one thread per output voxel, coalesced along x.  This translation unit is compiled with
+// -fmad=false: the double-precision expressions below are evaluated operation by operation, so that the density
+// handed to the accumulation stage is reproducible to the last bit.
+#include "internal.h"
+
+#include <cuda_runtime.h>
+
+namespace pbs4d {
+
+namespace {
+
+__device__ __forceinline__ double table_density(double hu, int n, const float* __restrict__ hp,
+                                                const float* __restrict__ rp)
+{
+    if (hu <= (double)hp[0]) return (double)rp[0];
+    if (hu >= (double)hp[n - 1]) return (double)rp[n - 1];
+    int k = 0;
+    while (k < n - 2 && hu >= (double)hp[k + 1]) ++k;
+    const double f = (hu - (double)hp[k]) / ((double)hp[k + 1] - (double)hp[k]);
+    return (double)rp[k] + f * ((double)rp[k + 1] - (double)rp[k]);
+}
+
+__global__ void hu_to_density_same_grid(long long nvox, const int16_t* __restrict__ hu, int n_pts,
+                                        const float* __restrict__ hp, const float* __restrict__ rp,
+                                        float* __restrict__ out)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride)
+        out[i] = (float)table_density((double)hu[i], n_pts, hp, rp);
+}
+
+// dose-grid voxel = overlap-volume-weighted mean of the densities of the CT voxels it intersects
+__global__ void hu_to_density_resample(pbs4d_grid ct, pbs4d_grid dg, const int16_t* __restrict__ hu, int n_pts,
+                                       const float* __restrict__ hp, const float* __restrict__ rp,
+                                       float* __restrict__ out)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= dg.nx || y >= dg.ny || z >= dg.nz) return;
+    const double ch[3] = { (double)ct.hx, (double)ct.hy, (double)ct.hz };
+    const double co[3] = { (double)ct.ox, (double)ct.oy, (double)ct.oz };
+    const int    cn[3] = { ct.nx, ct.ny, ct.nz };
+    const double dh[3] = { (double)dg.hx, (double)dg.hy, (double)dg.hz };
+    const double d0[3] = { (double)dg.ox, (double)dg.oy, (double)dg.oz };
+    const int    id[3] = { x, y, z };
+    int lo[3], hi[3]; double a[3], b[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        a[k] = d0[k] + (double)id[k] * dh[k];
+        b[k] = a[k] + dh[k];
+        lo[k] = max((int)floor((a[k] - co[k]) / ch[k]), 0);
+        hi[k] = min((int)ceil((b[k] - co[k]) / ch[k]), cn[k]);
+    }
+    double acc = 0.0, wsum = 0.0;
+    for (int kz = lo[2]; kz < hi[2]; ++kz)
+        for (int ky = lo[1]; ky < hi[1]; ++ky)
+            for (int kx = lo[0]; kx < hi[0]; ++kx) {
+                const int ic[3] = { kx, ky, kz };
+                double wv = 1.0;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double ca = co[k] + (double)ic[k] * ch[k], cb = ca + ch[k];
+                    const double ov = fmin(b[k], cb) - fmax(a[k], ca);
+                    wv *= ov > 0.0 ? ov : 0.0;
+                }
+                if (wv > 0.0) {
+                    acc  += wv * table_density((double)hu[((size_t)kz * cn[1] + ky) * cn[0] + kx], n_pts, hp, rp);
+                    wsum += wv;
+                }
+            }
+    out[((size_t)z * dg.ny + y) * dg.nx + x] = (float)(wsum > 0.0 ? acc / wsum : (double)rp[0]);
+}
+
+// a7 / T12: D = Q 2^-k 1.602176634e-10 / (rho V_cm3)  [Gy]; optionally per proton
+__global__ void finalize_dose_kernel(long long nvox, const float* __restrict__ rho, const long long* __restrict__ Q,
+                                     double inv_scale, double vol_cm3, double per_protons, float* __restrict__ dose)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride) {
+        double D = (double)Q[i] * inv_scale * 1.602176634e-10 / ((double)rho[i] * vol_cm3);
+        if (per_protons > 0.0) D /= per_protons;
+        dose[i] = (float)D;
+    }
+}
+
+}  // namespace
+
+void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
+                          const float* hp, const float* rp, float* rho_out, cudaStream_t st)
+{
+    if (!dose_grid) {
+        const long long nvox = (long long)ct.nx * ct.ny * ct.nz;
+        const int blocks = (int)min((nvox + 255) / 256, (long long)148 * 16);
+        hu_to_density_same_grid<<<blocks, 256, 0, st>>>(nvox, hu, n_pts, hp, rp, rho_out);
+    } else {
+        dim3 b(32, 8, 1), g((dose_grid->nx + 31) / 32, (dose_grid->ny + 7) / 8, dose_grid->nz);
+        hu_to_density_resample<<<g, b, 0, st>>>(ct, *dose_grid, hu, n_pts, hp, rp, rho_out);
+    }
+}
+
+void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long* Q, int32_t fixed_shift,
+                          double per_protons, float* dose, cudaStream_t st)
+{
+    const long long nvox = (long long)g.nx * g.ny * g.nz;
+    const double vol_cm3 = (double)g.hx * (double)g.hy * (double)g.hz * 1.0e-3;
+    const int blocks = (int)min((nvox + 255) / 256, (long long)148 * 16);
+    finalize_dose_kernel<<<blocks, 256, 0, st>>>(nvox, rho, Q, ldexp(1.0, -fixed_shift), vol_cm3, per_protons, dose);
+}
+
+}  // namespace pbs4d

@@ -1,0 +1,60 @@
+// Internal declarations shared by the translation units of libpbs4d (not part of the public boundary).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "pbs4d.h"
+
+#ifdef __CUDACC__
+#include <cuda_runtime.h>
+#else
+typedef struct CUstream_st* cudaStream_t;
+#endif
+
+namespace pbs4d {
+
+// ---- host delivery simulator (delivery.cpp) ----
+int simulate_delivery_host(const std::vector<pbs4d_field>& fields, const std::vector<pbs4d_spot>& spots,
+                           const pbs4d_delivery_params& prm, uint64_t total_histories,
+                           std::vector<pbs4d_segment>& segments, std::vector<int64_t>& field_time_ns,
+                           int64_t& dropped_protons, std::string& err);
+int32_t fixed_shift_for(const std::vector<pbs4d_segment>& segments, const std::vector<pbs4d_spot>& spots);
+
+// ---- device-side segment record (transport.cu): everything a history needs from its (field, spot) ----
+struct DevSegment {
+    float dir[3], eu[3], ev[3], ref[3];
+    float x_mm, y_mm, energy_mev, sigma_mm;
+    float weight_scaled;          // weight * 2^k as float (deposit -> quanta)
+    float pad0;
+    double weight_scaled_d;       // same in double, for the incident/escaped tallies
+    int64_t first_history;        // global Philox history index of local history 0
+    int64_t local_begin;          // index of its first history within the phase launch
+};
+
+struct TransportCounters {       // device tallies of one launch
+    unsigned long long histories, steps;
+    long long q_incident, q_deposited, q_escaped;
+};
+
+// Launchers (all asynchronous on `st`).
+void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, int32_t n_segs,
+                      int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q, TransportCounters* counters,
+                      int sm_count, cudaStream_t st);
+const void* transport_kernel_symbol();
+
+void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
+                          const float* hu_pts_dev, const float* rho_pts_dev, float* rho_out, cudaStream_t st);
+void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long* Q, int32_t fixed_shift,
+                          double per_protons, float* dose, cudaStream_t st);
+
+struct AccCounters { unsigned long long subvoxels, dropped_ref, dropped_dvf; };
+void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho, const pbs4d_grid& dvf_grid,
+                      const float* disp, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
+                      long long* E, long long* M, AccCounters* counters, cudaStream_t st);
+// out = (first ? dose_ref : out_acc) ... see accumulate.cu: ratio-and-add over all pushed phases, then mask.
+void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_dev,
+                          const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev, float* out,
+                          cudaStream_t st);
+
+}  // namespace pbs4d
