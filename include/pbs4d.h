@@ -120,6 +120,14 @@ int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags);
 int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
                             pbs4d_phase_lists* out);
 
+/* The same simulation without a context or a device (host only; used by CPU tests and tools).  Writes at most
+ * max_segs segments to segs_out (may be NULL to query), the segment count to *n_segs_out, per-field end times to
+ * field_time_ns[n_fields] (optional), dropped protons and the fixed-point shift (optional). */
+int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field* fields, int64_t n_spots,
+                                 const pbs4d_spot* spots, const pbs4d_delivery_params* prm, uint64_t total_histories,
+                                 pbs4d_segment* segs_out, int64_t max_segs, int64_t* n_segs_out,
+                                 int64_t* field_time_ns, int64_t* dropped_protons, int32_t* fixed_shift);
+
 /* a4-a7: Monte Carlo transport of all segments of `phase` on that phase's density grid.
  * dose_dev (optional) receives fp32 Gy [z][y][x] on the dose grid for the delivered protons (divided by
  * per_protons if > 0, e.g. "Gy per proton"); rho_dev (optional) receives the density grid (dose and

@@ -1,0 +1,256 @@
+"""Thin Python binding of libpbs4d.so (include/pbs4d.h): argument marshalling only.
+
+Every step of the path runs inside the library's CUDA kernels / host simulator; PyTorch supplies device memory
+(tensors) and the CUDA stream.  Method names equal the C entry points without the `pbs4d_` prefix.
+There is no CPU fallback: a missing library or a missing CUDA device raises RuntimeError.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libpbs4d.so")
+
+GRID_DT = np.dtype([("nx", "i4"), ("ny", "i4"), ("nz", "i4"), ("hx", "f4"), ("hy", "f4"), ("hz", "f4"),
+                    ("ox", "f4"), ("oy", "f4"), ("oz", "f4")])
+FIELD_DT = np.dtype([("dir", "f4", 3), ("eu", "f4", 3), ("ev", "f4", 3), ("ref", "f4", 3), ("start_phase", "i4")])
+SPOT_DT = np.dtype([("field", "i4"), ("layer", "i4"), ("x_mm", "f4"), ("y_mm", "f4"), ("energy_mev", "f4"),
+                    ("sigma_mm", "f4"), ("weight", "f4")])
+DELIV_DT = np.dtype([("n_phases", "i4"), ("period_ns", "i8"), ("protons_per_weight", "i8"), ("protons_per_s", "i8"),
+                     ("ns_per_um", "i4"), ("layer_switch_ns", "i8"), ("repaints", "i4"), ("gate_mask", "u4")],
+                    align=True)
+SEG_DT = np.dtype([("field", "i4"), ("phase", "i4"), ("spot", "i4"), ("pad", "i4"), ("protons", "i8"),
+                   ("first_history", "i8"), ("n_hist", "i8"), ("weight", "f8")])
+
+NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
+
+EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
+           "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
+           "pbs4d_mc_dose_phase", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
+           "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host"]
+
+
+class PhaseLists(C.Structure):
+    _fields_ = [("n_segments", C.c_int64), ("segments", C.c_void_p), ("n_fields", C.c_int32),
+                ("field_time_ns", C.POINTER(C.c_int64)), ("dropped_protons", C.c_int64), ("fixed_shift", C.c_int32)]
+
+
+class McStats(C.Structure):
+    _fields_ = [("histories", C.c_uint64), ("steps", C.c_uint64), ("q_incident", C.c_int64),
+                ("q_deposited", C.c_int64), ("q_escaped", C.c_int64), ("fixed_shift", C.c_int32), ("pad", C.c_int32),
+                ("kernel_ms", C.c_float)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_ if n != "pad"}
+
+
+class AccStats(C.Structure):
+    _fields_ = [("subvoxels", C.c_uint64), ("dropped_outside_ref", C.c_uint64), ("dropped_outside_dvf", C.c_uint64),
+                ("push_ms", C.c_float), ("finalize_ms", C.c_float)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def load():
+    """dlopen libpbs4d.so; fails loudly if it has not been built (python -m paper_1809_03927_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1809_03927_b200.build` "
+                               "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name in EXPORTS:
+            getattr(lib, name)                                   # AttributeError if a symbol is not exported
+        lib.pbs4d_last_error.restype = C.c_char_p
+        lib.pbs4d_last_error.argtypes = [C.c_void_p]
+        lib.pbs4d_destroy.restype = None
+        lib.pbs4d_destroy.argtypes = [C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _np(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _ptr_array(tensors):
+    arr = (C.c_void_p * len(tensors))()
+    for i, t in enumerate(tensors):
+        arr[i] = None if t is None else t.data_ptr()
+    return arr
+
+
+def simulate_delivery_host(fields, spots, prm, total_histories):
+    """Device-free entry: the host delivery simulator alone (same code path as Context.simulate_delivery)."""
+    lib = load()
+    f = np.ascontiguousarray(fields, FIELD_DT)
+    s = np.ascontiguousarray(spots, SPOT_DT)
+    p = np.ascontiguousarray(prm, DELIV_DT)
+    n = C.c_int64(0)
+    args = [C.c_int32(len(f)), _np(f), C.c_int64(len(s)), _np(s), _np(p), C.c_uint64(int(total_histories))]
+    rc = lib.pbs4d_simulate_delivery_host(*args, None, C.c_int64(0), C.byref(n), None, None, None)
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_simulate_delivery_host: error {rc}")
+    segs = np.zeros(n.value, SEG_DT)
+    times = np.zeros(len(f), np.int64)
+    dropped = C.c_int64(0)
+    shift = C.c_int32(0)
+    rc = lib.pbs4d_simulate_delivery_host(*args, _np(segs), C.c_int64(n.value), C.byref(n), _np(times),
+                                          C.byref(dropped), C.byref(shift))
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_simulate_delivery_host: error {rc}")
+    return dict(segments=segs, field_time_ns=times, dropped_protons=int(dropped.value), fixed_shift=int(shift.value))
+
+
+class Context:
+    """One pbs4d_ctx on a CUDA device, enqueueing on torch's current stream of that device."""
+
+    def __init__(self, device=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("pbs4d needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.lib = load()
+        self.h = C.c_void_p()
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        rc = self.lib.pbs4d_create(C.byref(self.h), C.c_int(device), C.c_void_p(stream))
+        if rc != 0:
+            raise RuntimeError(f"pbs4d_create failed with code {rc}")
+        self.dose_shape = None
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.pbs4d_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc != 0:
+            raise RuntimeError(f"pbs4d error {rc}: {self.lib.pbs4d_last_error(self.h).decode()}")
+
+    def _dev(self, t, dtype):
+        assert t.is_cuda and t.dtype == dtype and t.is_contiguous(), "expected a contiguous CUDA tensor of " + str(dtype)
+        return t
+
+    # ---- a1 ----
+    def set_ct_phases(self, ct_grid, hu, dose_grid=None, hu_pts=(-1000.0, 0.0, 1000.0), rho_pts=(0.001, 1.0, 1.6)):
+        t = self.torch
+        phases = [self._dev(hu[p], t.int16) for p in range(len(hu))]
+        ct = np.ascontiguousarray(ct_grid, GRID_DT)
+        dg = None if dose_grid is None else np.ascontiguousarray(dose_grid, GRID_DT)
+        hp, rp = np.asarray(hu_pts, np.float32), np.asarray(rho_pts, np.float32)
+        self._check(self.lib.pbs4d_set_ct_phases(self.h, C.c_int32(len(phases)), _np(ct), _ptr_array(phases),
+                                                 None if dg is None else _np(dg), C.c_int32(len(hp)), _np(hp), _np(rp)))
+        g = ct if dg is None else dg
+        self.dose_shape = (int(g["nz"][0]), int(g["ny"][0]), int(g["nx"][0]))
+        self.n_phases = len(phases)
+
+    def set_density_phases(self, dose_grid, rho):
+        t = self.torch
+        phases = [self._dev(rho[p], t.float32) for p in range(len(rho))]
+        g = np.ascontiguousarray(dose_grid, GRID_DT)
+        self._check(self.lib.pbs4d_set_density_phases(self.h, C.c_int32(len(phases)), _np(g), _ptr_array(phases)))
+        self.dose_shape = (int(g["nz"][0]), int(g["ny"][0]), int(g["nx"][0]))
+        self.n_phases = len(phases)
+
+    # ---- a2 ----
+    def set_dvf(self, src_phase, ref_phase, dvf_grid, disp):
+        g = np.ascontiguousarray(dvf_grid, GRID_DT)
+        self._dev(disp, self.torch.float32)
+        self._check(self.lib.pbs4d_set_dvf(self.h, C.c_int32(src_phase), C.c_int32(ref_phase), _np(g),
+                                           C.c_void_p(disp.data_ptr())))
+
+    def set_plan_spots(self, fields, spots):
+        f = np.ascontiguousarray(fields, FIELD_DT)
+        s = np.ascontiguousarray(spots, SPOT_DT)
+        self._check(self.lib.pbs4d_set_plan_spots(self.h, C.c_int32(len(f)), _np(f), C.c_int64(len(s)), _np(s)))
+
+    def set_mc_flags(self, flags):
+        self._check(self.lib.pbs4d_set_mc_flags(self.h, C.c_uint32(flags)))
+
+    # ---- a3 ----
+    def simulate_delivery(self, prm, total_histories):
+        p = np.ascontiguousarray(prm, DELIV_DT)
+        out = PhaseLists()
+        self._check(self.lib.pbs4d_simulate_delivery(self.h, _np(p), C.c_uint64(int(total_histories)), C.byref(out)))
+        segs = np.zeros(out.n_segments, SEG_DT)
+        if out.n_segments:
+            C.memmove(segs.ctypes.data, out.segments, segs.nbytes)
+        times = np.array([out.field_time_ns[i] for i in range(out.n_fields)], np.int64)
+        return dict(segments=segs, field_time_ns=times, dropped_protons=int(out.dropped_protons),
+                    fixed_shift=int(out.fixed_shift))
+
+    # ---- a4-a7 ----
+    def mc_dose_phase(self, phase, seed, per_protons=0.0, want_dose=True, want_rho=False):
+        t = self.torch
+        dose = t.empty(self.dose_shape, dtype=t.float32, device=self.device) if want_dose else None
+        rho = t.empty(self.dose_shape, dtype=t.float32, device=self.device) if want_rho else None
+        st = McStats()
+        self._check(self.lib.pbs4d_mc_dose_phase(self.h, C.c_int32(phase), C.c_uint64(int(seed)),
+                                                 C.c_double(float(per_protons)),
+                                                 C.c_void_p(dose.data_ptr() if want_dose else None),
+                                                 C.c_void_p(rho.data_ptr() if want_rho else None), C.byref(st)))
+        return dose, rho, st.as_dict()
+
+    def get_phase_energy(self, phase):
+        t = self.torch
+        q = t.empty(self.dose_shape, dtype=t.int64, device=self.device)
+        self._check(self.lib.pbs4d_get_phase_energy(self.h, C.c_int32(phase), C.c_void_p(q.data_ptr())))
+        return q
+
+    # ---- a8-a9 ----
+    def accumulate_subvoxel(self, ref_phase, ns_xyz, phase_doses=None):
+        t = self.torch
+        out = t.empty(self.dose_shape, dtype=t.float32, device=self.device)
+        ptrs = None
+        if phase_doses is not None:
+            ptrs = _ptr_array([None if d is None else self._dev(d, t.float32) for d in phase_doses])
+        st = AccStats()
+        self._check(self.lib.pbs4d_accumulate_subvoxel(self.h, C.c_int32(ref_phase), C.c_int32(ns_xyz[0]),
+                                                       C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), ptrs,
+                                                       C.c_void_p(out.data_ptr()), C.byref(st)))
+        return out, st.as_dict()
+
+    def get_accumulators(self, src_phase):
+        t = self.torch
+        E = t.empty(self.dose_shape, dtype=t.int64, device=self.device)
+        M = t.empty(self.dose_shape, dtype=t.int64, device=self.device)
+        self._check(self.lib.pbs4d_get_accumulators(self.h, C.c_int32(src_phase), C.c_void_p(E.data_ptr()),
+                                                    C.c_void_p(M.data_ptr())))
+        return E, M
+
+    # ---- whole path, host buffers ----
+    def run_plan_host(self, ct_grid, hu_host, dose_grid, dvf_grid, disp_host, ref_phase, fields, spots, prm,
+                      total_histories, seed, ns_xyz, out_host, hu_pts=(-1000.0, 0.0, 1000.0),
+                      rho_pts=(0.001, 1.0, 1.6)):
+        """hu_host: list of int16 numpy arrays (or pinned CPU tensors' numpy views); disp_host: list (None = no DVF);
+        out_host: float32 numpy array [z,y,x] written in place.  Returns (histories_run, seconds[4])."""
+        ct = np.ascontiguousarray(ct_grid, GRID_DT)
+        dg = None if dose_grid is None else np.ascontiguousarray(dose_grid, GRID_DT)
+        vg = None if dvf_grid is None else np.ascontiguousarray(dvf_grid, GRID_DT)
+        hp, rp = np.asarray(hu_pts, np.float32), np.asarray(rho_pts, np.float32)
+        n = len(hu_host)
+        hu_ptrs = (C.c_void_p * n)(*[a.ctypes.data for a in hu_host])
+        dp = None
+        if disp_host is not None:
+            dp = (C.c_void_p * n)(*[None if a is None else a.ctypes.data for a in disp_host])
+        f = np.ascontiguousarray(fields, FIELD_DT)
+        s = np.ascontiguousarray(spots, SPOT_DT)
+        p = np.ascontiguousarray(prm, DELIV_DT)
+        run = C.c_uint64(0)
+        secs = (C.c_double * 4)()
+        self._check(self.lib.pbs4d_run_plan_host(
+            self.h, C.c_int32(n), _np(ct), hu_ptrs, None if dg is None else _np(dg), C.c_int32(len(hp)), _np(hp),
+            _np(rp), None if vg is None else _np(vg), dp, C.c_int32(ref_phase), C.c_int32(len(f)), _np(f),
+            C.c_int64(len(s)), _np(s), _np(p), C.c_uint64(int(total_histories)), C.c_uint64(int(seed)),
+            C.c_int32(ns_xyz[0]), C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), _np(out_host), C.byref(run), secs))
+        g = ct if dg is None else dg
+        self.dose_shape = (int(g["nz"][0]), int(g["ny"][0]), int(g["nx"][0]))
+        return int(run.value), list(secs)

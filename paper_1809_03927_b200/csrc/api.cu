@@ -1,0 +1,521 @@
+// C-ABI boundary of libpbs4d (include/pbs4d.h): context, argument checks, device memory, launch sequencing.
+// No arithmetic of the method lives here -- it is in delivery.cpp (host, int64), transport.cu, grids.cu and
+// accumulate.cu (device).
+#include "internal.h"
+
+#include <cuda_runtime.h>
+
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <new>
+
+using namespace pbs4d;
+
+namespace {
+
+struct DevBuf {                          // RAII device allocation
+    void* p = nullptr; size_t bytes = 0;
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete; DevBuf& operator=(const DevBuf&) = delete;
+    ~DevBuf() { release(); }
+    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    cudaError_t ensure(size_t n) {
+        if (n <= bytes && p) return cudaSuccess;
+        release();
+        cudaError_t e = cudaMalloc(&p, n ? n : 1);
+        if (e == cudaSuccess) bytes = n;
+        return e;
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+struct PhaseLaunch {                     // per-phase segment table for the transport kernel
+    std::vector<DevSegment> segs;
+    int64_t n_hist = 0;
+    double protons = 0.0;
+};
+
+}  // namespace
+
+struct pbs4d_ctx {
+    int device = 0;
+    int sm_count = 148;
+    cudaStream_t stream = nullptr;
+    std::string err;
+
+    // geometry + densities (a1)
+    bool have_density = false;
+    int32_t n_phases = 0;
+    pbs4d_grid dose_grid{};
+    std::vector<std::unique_ptr<DevBuf>> rho;            // [phase] fp32 on dose grid
+    DevBuf table;                                        // hu_pts | rho_pts
+
+    // DVFs (a2)
+    struct Dvf { bool set = false; int32_t ref = -1; pbs4d_grid grid{}; std::unique_ptr<DevBuf> disp; };
+    std::vector<Dvf> dvf;                                // [src phase]
+
+    // plan (a2) and delivery (a3)
+    std::vector<pbs4d_field> fields;
+    std::vector<pbs4d_spot> spots;
+    bool have_delivery = false;
+    std::vector<pbs4d_segment> segments;
+    std::vector<int64_t> field_time;
+    int64_t dropped = 0;
+    int32_t fixed_shift = 40;
+    int32_t deliv_phases = 0;
+    std::vector<PhaseLaunch> launches;                   // [phase]
+    uint32_t mc_flags = 0;
+
+    // transport state (a4-a7)
+    std::vector<std::unique_ptr<DevBuf>> q;              // [phase] int64 energy grid
+    std::vector<std::unique_ptr<DevBuf>> dose;           // [phase] fp32 Gy
+    std::vector<bool> have_dose;
+    DevBuf seg_dev, counters;
+
+    // accumulation state (a8-a9)
+    std::vector<std::unique_ptr<DevBuf>> accE, accM;     // [phase]
+    std::vector<bool> have_acc;
+    DevBuf acc_counters;
+
+    size_t nvox() const { return (size_t)dose_grid.nx * dose_grid.ny * dose_grid.nz; }
+};
+
+namespace {
+
+int fail(pbs4d_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+
+int cuda_fail(pbs4d_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, e == cudaErrorMemoryAllocation ? PBS4D_ERR_NOMEM : PBS4D_ERR_CUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
+
+bool grid_ok(const pbs4d_grid* g)
+{
+    return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->hx > 0.0f && g->hy > 0.0f && g->hz > 0.0f &&
+           std::isfinite(g->ox) && std::isfinite(g->oy) && std::isfinite(g->oz) &&
+           (double)g->nx * g->ny * g->nz < 2.0e9;
+}
+
+void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
+{
+    ctx->n_phases = n_phases; ctx->dose_grid = g;
+    ctx->rho.clear(); ctx->q.clear(); ctx->dose.clear(); ctx->accE.clear(); ctx->accM.clear(); ctx->dvf.clear();
+    for (int p = 0; p < n_phases; ++p) {
+        ctx->rho.emplace_back(new DevBuf); ctx->q.emplace_back(new DevBuf); ctx->dose.emplace_back(new DevBuf);
+        ctx->accE.emplace_back(new DevBuf); ctx->accM.emplace_back(new DevBuf);
+    }
+    ctx->dvf.resize(n_phases);
+    ctx->have_dose.assign(n_phases, false);
+    ctx->have_acc.assign(n_phases, false);
+    ctx->have_density = false;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return PBS4D_ERR_ARG;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) return PBS4D_ERR_CUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return PBS4D_ERR_CUDA;
+    pbs4d_ctx* ctx = new (std::nothrow) pbs4d_ctx;
+    if (!ctx) return PBS4D_ERR_NOMEM;
+    ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaDeviceProp prop{};
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) ctx->sm_count = prop.multiProcessorCount;
+    *out = ctx;
+    return PBS4D_OK;
+}
+
+void pbs4d_destroy(pbs4d_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    delete ctx;
+}
+
+const char* pbs4d_last_error(const pbs4d_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_dev,
+                        const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_dev || (dose_grid && !grid_ok(dose_grid)) ||
+        n_pts < 2 || n_pts > 64 || !hu_pts || !rho_pts)
+        return fail(ctx, PBS4D_ERR_ARG, "set_ct_phases: bad argument");
+    for (int i = 0; i < n_pts; ++i) {
+        if (!(rho_pts[i] > 0.0f) || (i && !(hu_pts[i] > hu_pts[i - 1])))
+            return fail(ctx, PBS4D_ERR_ARG, "set_ct_phases: table must ascend in HU with positive densities");
+    }
+    for (int p = 0; p < n_phases; ++p) if (!hu_dev[p]) return fail(ctx, PBS4D_ERR_ARG, "set_ct_phases: null phase");
+    CU(cudaSetDevice(ctx->device));
+    const pbs4d_grid& g = dose_grid ? *dose_grid : *ct;
+    reset_phase_state(ctx, n_phases, g);
+    CU(ctx->table.ensure(2 * n_pts * sizeof(float)));
+    CU(cudaMemcpyAsync(ctx->table.p, hu_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->table.as<float>() + n_pts, rho_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice,
+                       ctx->stream));
+    for (int p = 0; p < n_phases; ++p) {
+        CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
+        launch_hu_to_density(*ct, hu_dev[p], dose_grid, n_pts, ctx->table.as<float>(),
+                             ctx->table.as<float>() + n_pts, ctx->rho[p]->as<float>(), ctx->stream);
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_density = true;
+    return PBS4D_OK;
+}
+
+int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* dose_grid,
+                             const float* const* rho_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (n_phases < 1 || n_phases > 32 || !grid_ok(dose_grid) || !rho_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: bad argument");
+    for (int p = 0; p < n_phases; ++p) if (!rho_dev[p]) return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: null phase");
+    CU(cudaSetDevice(ctx->device));
+    reset_phase_state(ctx, n_phases, *dose_grid);
+    for (int p = 0; p < n_phases; ++p) {
+        CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
+        CU(cudaMemcpyAsync(ctx->rho[p]->p, rho_dev[p], ctx->nvox() * sizeof(float), cudaMemcpyDeviceToDevice,
+                           ctx->stream));
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_density = true;
+    return PBS4D_OK;
+}
+
+int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
+                  const float* disp_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "set_dvf: call set_ct_phases/set_density_phases first");
+    if (src_phase < 0 || src_phase >= ctx->n_phases || ref_phase < 0 || ref_phase >= ctx->n_phases ||
+        src_phase == ref_phase || !grid_ok(dvf_grid) || !disp_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "set_dvf: bad argument");
+    CU(cudaSetDevice(ctx->device));
+    auto& d = ctx->dvf[src_phase];
+    if (!d.disp) d.disp.reset(new DevBuf);
+    const size_t bytes = (size_t)3 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
+    CU(d.disp->ensure(bytes));
+    CU(cudaMemcpyAsync(d.disp->p, disp_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
+    return PBS4D_OK;
+}
+
+int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fields,
+                         int64_t n_spots, const pbs4d_spot* spots)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (n_fields < 1 || !fields || n_spots < 1 || !spots) return fail(ctx, PBS4D_ERR_ARG, "set_plan_spots: bad argument");
+    for (int64_t s = 0; s < n_spots; ++s) {
+        const pbs4d_spot& sp = spots[s];
+        if (sp.field < 0 || sp.field >= n_fields || !(sp.energy_mev > 0.5f) || !(sp.energy_mev < 500.0f) ||
+            !(sp.sigma_mm >= 0.0f) || !(sp.weight >= 0.0f) || !std::isfinite(sp.x_mm) || !std::isfinite(sp.y_mm))
+            return fail(ctx, PBS4D_ERR_ARG, "set_plan_spots: bad spot " + std::to_string(s));
+    }
+    for (int32_t f = 0; f < n_fields; ++f) {
+        const float* d = fields[f].dir;
+        const float n2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+        if (!(std::fabs(n2 - 1.0f) < 1e-3f) || fields[f].start_phase < 0)
+            return fail(ctx, PBS4D_ERR_ARG, "set_plan_spots: field direction must be a unit vector, start_phase >= 0");
+    }
+    ctx->fields.assign(fields, fields + n_fields);
+    ctx->spots.assign(spots, spots + n_spots);
+    ctx->have_delivery = false;
+    return PBS4D_OK;
+}
+
+int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    ctx->mc_flags = flags;
+    return PBS4D_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------
+// a3: delivery simulation (host) and per-phase launch tables
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
+                                       pbs4d_phase_lists* out)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: null parameters");
+    if (ctx->fields.empty()) return fail(ctx, PBS4D_ERR_ORDER, "simulate_delivery: call set_plan_spots first");
+    if (total_histories > (uint64_t)1 << 62) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: too many histories");
+    std::string err;
+    int rc = simulate_delivery_host(ctx->fields, ctx->spots, *prm, total_histories, ctx->segments, ctx->field_time,
+                                    ctx->dropped, err);
+    if (rc != PBS4D_OK) return fail(ctx, rc, "simulate_delivery: " + err);
+    ctx->fixed_shift = fixed_shift_for(ctx->segments, ctx->spots);
+    ctx->deliv_phases = prm->n_phases;
+
+    // overflow guard: total quanta of the plan must stay below 2^62
+    double tot = 0.0;
+    for (const auto& sg : ctx->segments) tot += (double)sg.protons * (double)ctx->spots[sg.spot].energy_mev;
+    if (std::ldexp(tot * 1.1, ctx->fixed_shift) > 4611686018427387904.0)
+        return fail(ctx, PBS4D_ERR_OVERFLOW, "simulate_delivery: plan energy does not fit the fixed-point range");
+
+    // per-phase launch tables: one DevSegment per segment with histories, local_begin = running history count
+    ctx->launches.assign(prm->n_phases, PhaseLaunch{});
+    const double scale = std::ldexp(1.0, ctx->fixed_shift);
+    for (const auto& sg : ctx->segments) {
+        PhaseLaunch& L = ctx->launches[sg.phase];
+        L.protons += (double)sg.protons;
+        if (sg.n_hist <= 0) continue;
+        const pbs4d_field& f = ctx->fields[sg.field];
+        const pbs4d_spot&  s = ctx->spots[sg.spot];
+        DevSegment d{};
+        for (int k = 0; k < 3; ++k) { d.dir[k] = f.dir[k]; d.eu[k] = f.eu[k]; d.ev[k] = f.ev[k]; d.ref[k] = f.ref[k]; }
+        d.x_mm = s.x_mm; d.y_mm = s.y_mm; d.energy_mev = s.energy_mev; d.sigma_mm = s.sigma_mm;
+        d.weight_scaled_d = sg.weight * scale;
+        d.weight_scaled   = (float)d.weight_scaled_d;
+        d.first_history   = sg.first_history;
+        d.local_begin     = L.n_hist;
+        L.segs.push_back(d);
+        L.n_hist += sg.n_hist;
+    }
+    ctx->have_delivery = true;
+    std::fill(ctx->have_dose.begin(), ctx->have_dose.end(), false);
+    if (out) {
+        out->n_segments = (int64_t)ctx->segments.size();
+        out->segments = ctx->segments.data();
+        out->n_fields = (int32_t)ctx->field_time.size();
+        out->field_time_ns = ctx->field_time.data();
+        out->dropped_protons = ctx->dropped;
+        out->fixed_shift = ctx->fixed_shift;
+    }
+    return PBS4D_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a4-a7: transport + scoring + finalize for one phase
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
+                                   float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phase: no densities (set_ct_phases)");
+    if (!ctx->have_delivery) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phase: call simulate_delivery first");
+    if (phase < 0 || phase >= ctx->n_phases || phase >= ctx->deliv_phases)
+        return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phase: phase out of range");
+    CU(cudaSetDevice(ctx->device));
+    const size_t nvox = ctx->nvox();
+    PhaseLaunch& L = ctx->launches[phase];
+    CU(ctx->q[phase]->ensure(nvox * sizeof(long long)));
+    CU(ctx->dose[phase]->ensure(nvox * sizeof(float)));
+    CU(ctx->counters.ensure(sizeof(TransportCounters)));
+    CU(cudaMemsetAsync(ctx->q[phase]->p, 0, nvox * sizeof(long long), ctx->stream));
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(TransportCounters), ctx->stream));
+    float ms = 0.0f;
+    if (L.n_hist > 0) {
+        CU(ctx->seg_dev.ensure(L.segs.size() * sizeof(DevSegment)));
+        CU(cudaMemcpyAsync(ctx->seg_dev.p, L.segs.data(), L.segs.size() * sizeof(DevSegment), cudaMemcpyHostToDevice,
+                           ctx->stream));
+        cudaEvent_t e0, e1;
+        CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+        CU(cudaEventRecord(e0, ctx->stream));
+        launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->seg_dev.as<DevSegment>(),
+                         (int32_t)L.segs.size(), L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
+                         ctx->counters.as<TransportCounters>(), ctx->sm_count, ctx->stream);
+        CU(cudaEventRecord(e1, ctx->stream));
+        CU(cudaGetLastError());
+        CU(cudaEventSynchronize(e1));
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+    }
+    launch_finalize_dose(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->q[phase]->as<long long>(),
+                         ctx->fixed_shift, per_protons, ctx->dose[phase]->as<float>(), ctx->stream);
+    CU(cudaGetLastError());
+    if (dose_dev) CU(cudaMemcpyAsync(dose_dev, ctx->dose[phase]->p, nvox * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (rho_dev)  CU(cudaMemcpyAsync(rho_dev, ctx->rho[phase]->p, nvox * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    TransportCounters tc{};
+    CU(cudaMemcpyAsync(&tc, ctx->counters.p, sizeof(tc), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_dose[phase] = true;
+    if (stats) {
+        stats->histories = tc.histories; stats->steps = tc.steps;
+        stats->q_incident = tc.q_incident; stats->q_deposited = tc.q_deposited; stats->q_escaped = tc.q_escaped;
+        stats->fixed_shift = ctx->fixed_shift; stats->pad = 0; stats->kernel_ms = ms;
+    }
+    return PBS4D_OK;
+}
+
+extern "C" int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (phase < 0 || phase >= ctx->n_phases || !q_dev) return fail(ctx, PBS4D_ERR_ARG, "get_phase_energy: bad argument");
+    if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "get_phase_energy: mc_dose_phase not run for this phase");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaMemcpyAsync(q_dev, ctx->q[phase]->p, ctx->nvox() * sizeof(long long), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return PBS4D_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a8-a9: subvoxel energy/mass push of every source phase with a DVF to ref_phase, then ratio + sum + mask
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                                         const float* const* phase_dose_dev, float* dose4d_dev,
+                                         pbs4d_acc_stats* stats)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_subvoxel: no densities");
+    if (ref_phase < 0 || ref_phase >= ctx->n_phases || nsx < 1 || nsy < 1 || nsz < 1 || nsx > 64 || nsy > 64 ||
+        nsz > 64 || !dose4d_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "accumulate_subvoxel: bad argument");
+    auto dose_of = [&](int p) -> const float* {
+        if (phase_dose_dev) return phase_dose_dev[p];
+        return ctx->have_dose[p] ? ctx->dose[p]->as<float>() : nullptr;
+    };
+    if (!dose_of(ref_phase)) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_subvoxel: no dose for the reference phase");
+    std::vector<int> src;
+    for (int p = 0; p < ctx->n_phases; ++p)
+        if (p != ref_phase && ctx->dvf[p].set && ctx->dvf[p].ref == ref_phase && dose_of(p)) src.push_back(p);
+    if (src.size() > 32) return fail(ctx, PBS4D_ERR_ARG, "accumulate_subvoxel: more than 32 source phases");
+    CU(cudaSetDevice(ctx->device));
+    const size_t nvox = ctx->nvox();
+    CU(ctx->acc_counters.ensure(sizeof(AccCounters)));
+    CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
+    cudaEvent_t e0, e1, e2;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1)); CU(cudaEventCreate(&e2));
+    std::fill(ctx->have_acc.begin(), ctx->have_acc.end(), false);
+    for (int p : src) {
+        CU(ctx->accE[p]->ensure(nvox * sizeof(long long)));
+        CU(ctx->accM[p]->ensure(nvox * sizeof(long long)));
+        CU(cudaMemsetAsync(ctx->accE[p]->p, 0, nvox * sizeof(long long), ctx->stream));
+        CU(cudaMemsetAsync(ctx->accM[p]->p, 0, nvox * sizeof(long long), ctx->stream));
+    }
+    CU(cudaEventRecord(e0, ctx->stream));
+    std::vector<const long long*> Ep, Mp; std::vector<pbs4d_grid> dg;
+    for (int p : src) {
+        launch_emtm_push(ctx->dose_grid, dose_of(p), ctx->rho[p]->as<float>(), ctx->dvf[p].grid,
+                         ctx->dvf[p].disp->as<float>(), ctx->dose_grid, nsx, nsy, nsz,
+                         ctx->accE[p]->as<long long>(), ctx->accM[p]->as<long long>(),
+                         ctx->acc_counters.as<AccCounters>(), ctx->stream);
+        Ep.push_back(ctx->accE[p]->as<long long>()); Mp.push_back(ctx->accM[p]->as<long long>());
+        dg.push_back(ctx->dvf[p].grid);
+        ctx->have_acc[p] = true;
+    }
+    CU(cudaEventRecord(e1, ctx->stream));
+    launch_emtm_finalize(ctx->dose_grid, dose_of(ref_phase), (int)src.size(), Ep.data(), Mp.data(), dg.data(),
+                         dose4d_dev, ctx->stream);
+    CU(cudaEventRecord(e2, ctx->stream));
+    CU(cudaGetLastError());
+    AccCounters ac{};
+    CU(cudaMemcpyAsync(&ac, ctx->acc_counters.p, sizeof(ac), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (stats) {
+        stats->subvoxels = (uint64_t)src.size() * nvox * nsx * nsy * nsz;
+        stats->dropped_outside_ref = ac.dropped_ref; stats->dropped_outside_dvf = ac.dropped_dvf;
+        cudaEventElapsedTime(&stats->push_ms, e0, e1);
+        cudaEventElapsedTime(&stats->finalize_ms, e1, e2);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
+    return PBS4D_OK;
+}
+
+extern "C" int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (src_phase < 0 || src_phase >= ctx->n_phases || !e_dev || !m_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "get_accumulators: bad argument");
+    if (!ctx->have_acc[src_phase]) return fail(ctx, PBS4D_ERR_ORDER, "get_accumulators: phase was not pushed");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaMemcpyAsync(e_dev, ctx->accE[src_phase]->p, ctx->nvox() * sizeof(long long), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(m_dev, ctx->accM[src_phase]->p, ctx->nvox() * sizeof(long long), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return PBS4D_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// whole path with host buffers (end-to-end entry used by bench.py's e2e leg)
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_host,
+                                   const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts,
+                                   const pbs4d_grid* dvf_grid, const float* const* disp_host, int32_t ref_phase,
+                                   int32_t n_fields, const pbs4d_field* fields, int64_t n_spots, const pbs4d_spot* spots,
+                                   const pbs4d_delivery_params* prm, uint64_t total_histories, uint64_t seed,
+                                   int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
+                                   double* seconds)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_host || !prm || !dose4d_host || ref_phase < 0 ||
+        ref_phase >= n_phases || prm->n_phases != n_phases || (disp_host && !grid_ok(dvf_grid)))
+        return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: bad argument");
+    using clk = std::chrono::steady_clock;
+    auto sec = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
+    CU(cudaSetDevice(ctx->device));
+    const auto t0 = clk::now();
+
+    // H2D: CT phases -> densities, DVFs
+    const size_t ct_vox = (size_t)ct->nx * ct->ny * ct->nz;
+    DevBuf hu_dev;
+    CU(hu_dev.ensure((size_t)n_phases * ct_vox * sizeof(int16_t)));
+    std::vector<const int16_t*> hu_ptrs(n_phases);
+    for (int p = 0; p < n_phases; ++p) {
+        if (!hu_host[p]) return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: null CT phase");
+        hu_ptrs[p] = hu_dev.as<int16_t>() + (size_t)p * ct_vox;
+        CU(cudaMemcpyAsync((void*)hu_ptrs[p], hu_host[p], ct_vox * sizeof(int16_t), cudaMemcpyHostToDevice, ctx->stream));
+    }
+    int rc = pbs4d_set_ct_phases(ctx, n_phases, ct, hu_ptrs.data(), dose_grid, n_pts, hu_pts, rho_pts);
+    if (rc != PBS4D_OK) return rc;
+    hu_dev.release();
+    if (disp_host) {
+        const size_t dvf_bytes = (size_t)3 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
+        DevBuf tmp;
+        for (int p = 0; p < n_phases; ++p) {
+            if (p == ref_phase || !disp_host[p]) continue;
+            CU(tmp.ensure(dvf_bytes));
+            CU(cudaMemcpyAsync(tmp.p, disp_host[p], dvf_bytes, cudaMemcpyHostToDevice, ctx->stream));
+            rc = pbs4d_set_dvf(ctx, p, ref_phase, dvf_grid, tmp.as<float>());
+            if (rc != PBS4D_OK) return rc;
+        }
+    }
+    const auto t1 = clk::now();
+
+    rc = pbs4d_set_plan_spots(ctx, n_fields, fields, n_spots, spots);
+    if (rc != PBS4D_OK) return rc;
+    rc = pbs4d_simulate_delivery(ctx, prm, total_histories, nullptr);
+    if (rc != PBS4D_OK) return rc;
+    const auto t2 = clk::now();
+
+    uint64_t run = 0;
+    for (int p = 0; p < n_phases; ++p) {
+        if (ctx->launches[p].n_hist <= 0 && p != ref_phase) continue;
+        pbs4d_mc_stats st{};
+        rc = pbs4d_mc_dose_phase(ctx, p, seed, 0.0, nullptr, nullptr, &st);
+        if (rc != PBS4D_OK) return rc;
+        run += st.histories;
+    }
+    const auto t3 = clk::now();
+
+    DevBuf out;
+    CU(out.ensure(ctx->nvox() * sizeof(float)));
+    rc = pbs4d_accumulate_subvoxel(ctx, ref_phase, nsx, nsy, nsz, nullptr, out.as<float>(), nullptr);
+    if (rc != PBS4D_OK) return rc;
+    CU(cudaMemcpyAsync(dose4d_host, out.p, ctx->nvox() * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    const auto t4 = clk::now();
+    if (histories_run) *histories_run = run;
+    if (seconds) { seconds[0] = sec(t0, t1); seconds[1] = sec(t1, t2); seconds[2] = sec(t2, t3); seconds[3] = sec(t3, t4); }
+    return PBS4D_OK;
+}

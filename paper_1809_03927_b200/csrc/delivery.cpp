@@ -145,3 +145,27 @@ int32_t fixed_shift_for(const std::vector<pbs4d_segment>& segments, const std::v
 }
 
 }  // namespace pbs4d
+
+extern "C" int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field* fields, int64_t n_spots,
+                                            const pbs4d_spot* spots, const pbs4d_delivery_params* prm,
+                                            uint64_t total_histories, pbs4d_segment* segs_out, int64_t max_segs,
+                                            int64_t* n_segs_out, int64_t* field_time_ns, int64_t* dropped_protons,
+                                            int32_t* fixed_shift)
+{
+    if (n_fields < 1 || !fields || n_spots < 1 || !spots || !prm || !n_segs_out) return PBS4D_ERR_ARG;
+    std::vector<pbs4d_field> f(fields, fields + n_fields);
+    std::vector<pbs4d_spot> s(spots, spots + n_spots);
+    for (const auto& sp : s) if (sp.field < 0 || sp.field >= n_fields) return PBS4D_ERR_ARG;
+    std::vector<pbs4d_segment> segs; std::vector<int64_t> times; int64_t dropped = 0; std::string err;
+    const int rc = pbs4d::simulate_delivery_host(f, s, *prm, total_histories, segs, times, dropped, err);
+    if (rc != PBS4D_OK) return rc;
+    *n_segs_out = (int64_t)segs.size();
+    if (segs_out) {
+        if (max_segs < (int64_t)segs.size()) return PBS4D_ERR_ARG;
+        std::copy(segs.begin(), segs.end(), segs_out);
+    }
+    if (field_time_ns) std::copy(times.begin(), times.end(), field_time_ns);
+    if (dropped_protons) *dropped_protons = dropped;
+    if (fixed_shift) *fixed_shift = pbs4d::fixed_shift_for(segs, s);
+    return PBS4D_OK;
+}
