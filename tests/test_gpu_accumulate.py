@@ -1,0 +1,138 @@
+"""GPU parity: EMTM subvoxel accumulation and density kernels vs the oracle -- BIT-EXACT (BASELINE.json north_star:
+"accumulation and delivery binning must be bit-exact, which the fixed-point atomics make possible")."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as orc
+from paper_1809_03927_b200 import binding, build, synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    build.build()
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def gpu_accumulate(ctx, c, ns, phases=None, dvf_grids=None):
+    P = len(c["doses"])
+    rho = torch.from_numpy(c["rhos"]).cuda()
+    dose = torch.from_numpy(c["doses"]).cuda()
+    ctx.set_density_phases(c["grid"], [rho[p] for p in range(P)])
+    keep = []
+    for p in range(P):
+        if c["disps"][p] is None or (phases is not None and p not in phases):
+            continue
+        d = torch.from_numpy(c["disps"][p]).cuda()
+        ctx.set_dvf(p, c["ref_phase"], c["dvf_grid"] if dvf_grids is None else dvf_grids[p], d)
+        keep.append(p)
+    out, st = ctx.accumulate_subvoxel(c["ref_phase"], ns, [dose[p] for p in range(P)])
+    EM = {p: tuple(t.cpu().numpy() for t in ctx.get_accumulators(p)) for p in keep}
+    return out.cpu().numpy(), st, EM
+
+
+def oracle_accumulate(c, ns, phases=None, dvf_grids=None):
+    P = len(c["doses"])
+    disps = [c["disps"][p] if (phases is None or p in phases) else None for p in range(P)]
+    grids = [c["dvf_grid"] if dvf_grids is None else dvf_grids[p] for p in range(P)]
+    EM = {}
+    for p in range(P):
+        if disps[p] is not None:
+            E, M, _ = orc.emtm_push(c["grid"], c["doses"][p], c["rhos"][p], grids[p], disps[p], c["grid"], ns)
+            EM[p] = (E, M)
+    out, st = orc.accumulate_subvoxel(c["grid"], c["doses"], c["rhos"], disps, grids, c["ref_phase"], ns)
+    return out, st, EM
+
+
+def assert_bit_exact(g, o):
+    out_g, st_g, EM_g = g
+    out_o, st_o, EM_o = o
+    assert set(EM_g) == set(EM_o)
+    for p in EM_o:
+        assert (EM_g[p][0] == EM_o[p][0]).all(), f"E differs, phase {p}"
+        assert (EM_g[p][1] == EM_o[p][1]).all(), f"M differs, phase {p}"
+    assert out_g.view(np.uint32).tobytes() == out_o.view(np.uint32).tobytes()
+    for k in ("subvoxels", "dropped_outside_ref", "dropped_outside_dvf"):
+        assert st_g[k] == int(st_o[k]), k
+
+
+@pytest.mark.parametrize("ns", [(1, 1, 1), (2, 2, 2), (3, 3, 3), (4, 4, 4), (2, 2, 5)])
+def test_config4_small_bit_exact(ctx, ns):
+    # 44^3: several 32x8 tiles with ragged tails in x and y
+    c = synth.config4(n=44, n_phases=4)
+    assert_bit_exact(gpu_accumulate(ctx, c, ns), oracle_accumulate(c, ns))
+
+
+def test_coarse_and_partial_dvf_grid(ctx):
+    # DVF on a coarser grid (paper Table I: deformation grids ~2x coarser than the CT) that does not cover the dose
+    # grid: exercises clamp-to-edge, the outside-DVF drop and the coverage mask
+    c = synth.config4(n=40, n_phases=3, dvf_div=2)
+    dg = c["dvf_grid"].copy()
+    dg["ox"], dg["oy"], dg["oz"] = 6.0, 3.0, 9.0
+    grids = [dg, dg, dg]
+    g = gpu_accumulate(ctx, c, (2, 2, 2), dvf_grids=grids)
+    o = oracle_accumulate(c, (2, 2, 2), dvf_grids=grids)
+    assert_bit_exact(g, o)
+    assert g[1]["dropped_outside_dvf"] > 0 and g[1]["dropped_outside_ref"] > 0
+    assert (g[0] == 0).any() and (g[0] != 0).any()
+
+
+def test_anisotropic_voxels(ctx):
+    c = synth.config4(n=36, n_phases=3)
+    for name in ("grid", "dvf_grid"):
+        c[name] = c[name].copy()
+        c[name]["hx"], c[name]["hy"], c[name]["hz"] = 0.98, 0.98, 2.5
+        c[name]["ox"], c[name]["oy"], c[name]["oz"] = -17.3, 4.1, 100.0
+    for p in range(1, 3):
+        c["disps"][p] = (c["disps"][p] * 0.3).astype(np.float32)
+    assert_bit_exact(gpu_accumulate(ctx, c, (2, 2, 5)), oracle_accumulate(c, (2, 2, 5)))
+
+
+def test_identity_dvf_is_the_plain_sum(ctx):
+    # identity DVF must reproduce the 3D static sum
+    c = synth.config4(n=33, n_phases=3)
+    for p in range(1, 3):
+        c["disps"][p] = np.zeros_like(c["disps"][p])
+    out, st, _ = gpu_accumulate(ctx, c, (2, 2, 2))
+    assert np.abs(out - c["doses"].astype(np.float64).sum(0)).max() < 1e-6 * 6
+    assert st["dropped_outside_ref"] == 0 and st["dropped_outside_dvf"] == 0
+
+
+def test_config4_full_size(ctx):
+    # BASELINE.json config 4: 10 phases of 128^3 at 2 mm; n = 2 and 4 over all phases; n = 8 on one source phase
+    c = synth.config4()
+    for ns in [(2, 2, 2), (4, 4, 4)]:
+        assert_bit_exact(gpu_accumulate(ctx, c, ns), oracle_accumulate(c, ns))
+    assert_bit_exact(gpu_accumulate(ctx, c, (8, 8, 8), phases=[3]), oracle_accumulate(c, (8, 8, 8), phases=[3]))
+
+
+def test_density_kernels_bit_exact(ctx):
+    for cfg in (synth.config2(), synth.config3(div=4, n_hist=10), synth.config5(div=8, n_hist=10)):
+        hu = torch.from_numpy(cfg["hu"]).cuda()
+        ctx.set_ct_phases(cfg["ct_grid"], [hu[p] for p in range(hu.shape[0])], cfg["dose_grid"])
+        ctx.set_plan_spots(cfg["fields"], cfg["spots"])
+        ctx.simulate_delivery(cfg["deliv"], 10)
+        for p in (0, hu.shape[0] - 1):
+            _, rho, _ = ctx.mc_dose_phase(p, 1, want_dose=False, want_rho=True)
+            want = orc.hu_to_density(cfg["ct_grid"], cfg["hu"][p], cfg["dose_grid"])
+            assert (rho.cpu().numpy() == want).all()
+
+
+def test_call_order_and_argument_errors(ctx):
+    c = synth.config4(n=16, n_phases=2)
+    fresh = binding.Context(0)
+    with pytest.raises(RuntimeError, match="-2"):
+        fresh.set_dvf(1, 0, c["dvf_grid"], torch.from_numpy(c["disps"][1]).cuda())
+    rho = torch.from_numpy(c["rhos"]).cuda()
+    fresh.set_density_phases(c["grid"], [rho[0], rho[1]])
+    with pytest.raises(RuntimeError, match="-1"):
+        fresh.set_dvf(1, 1, c["dvf_grid"], torch.from_numpy(c["disps"][1]).cuda())
+    with pytest.raises(RuntimeError, match="-2"):
+        fresh.accumulate_subvoxel(0, (2, 2, 2))                      # no doses yet
+    with pytest.raises(RuntimeError, match="-2"):
+        fresh.mc_dose_phase(0, 1)                                    # no delivery yet
+    fresh.close()
