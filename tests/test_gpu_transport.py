@@ -163,6 +163,8 @@ def test_empty_phase_and_resampled_grid(ctx):
     # config-3-like: CT 1x1x2.5 mm resampled to a 2 mm dose grid (reading A19); gated so that some phases are empty
     cfg = synth.config3(div=4, n_hist=200_000)
     cfg["deliv"]["gate_mask"] = 0b0000110000
+    cfg["deliv"]["period_ns"] = 500_000_000          # 50 ms phases: layers straddle phases 4 and 5
+    cfg["deliv"]["layer_switch_ns"] = 130_000_000
     g, dg = gpu_run(ctx, cfg, phases=[0, 4, 5])
     o, do = oracle_run(cfg, phases=[0, 4, 5])
     assert dg["segments"].tobytes() == np.ascontiguousarray(do["segments"]).tobytes()
