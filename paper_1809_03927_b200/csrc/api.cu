@@ -34,6 +34,7 @@ struct DevBuf {                          // RAII device allocation
 
 struct PhaseLaunch {                     // per-phase segment table for the transport kernel
     std::vector<DevSegment> segs;
+    std::vector<long long> seg_begin;    // segs[i].local_begin, contiguous for the kernel's binary search
     int64_t n_hist = 0;
     double protons = 0.0;
 };
@@ -291,6 +292,7 @@ extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_para
         d.first_history   = sg.first_history;
         d.local_begin     = L.n_hist;
         L.segs.push_back(d);
+        L.seg_begin.push_back(d.local_begin);
         L.n_hist += sg.n_hist;
     }
     ctx->have_delivery = true;
@@ -327,14 +329,16 @@ extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed,
     CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(TransportCounters), ctx->stream));
     float ms = 0.0f;
     if (L.n_hist > 0) {
-        CU(ctx->seg_dev.ensure(L.segs.size() * sizeof(DevSegment)));
-        CU(cudaMemcpyAsync(ctx->seg_dev.p, L.segs.data(), L.segs.size() * sizeof(DevSegment), cudaMemcpyHostToDevice,
-                           ctx->stream));
+        const size_t seg_bytes = L.segs.size() * sizeof(DevSegment);
+        CU(ctx->seg_dev.ensure(seg_bytes + L.segs.size() * sizeof(long long)));
+        CU(cudaMemcpyAsync(ctx->seg_dev.p, L.segs.data(), seg_bytes, cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->seg_dev.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
+                           cudaMemcpyHostToDevice, ctx->stream));
         cudaEvent_t e0, e1;
         CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
         CU(cudaEventRecord(e0, ctx->stream));
         launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->seg_dev.as<DevSegment>(),
-                         (int32_t)L.segs.size(), L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
+                         reinterpret_cast<const long long*>(ctx->seg_dev.as<char>() + seg_bytes), (int32_t)L.segs.size(), L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
                          ctx->counters.as<TransportCounters>(), ctx->sm_count, ctx->stream);
         CU(cudaEventRecord(e1, ctx->stream));
         CU(cudaGetLastError());

@@ -32,15 +32,16 @@ struct DevSegment {
     int64_t local_begin;          // index of its first history within the phase launch
 };
 
-struct TransportCounters {       // device tallies of one launch
+struct TransportCounters {       // device tallies of one launch (zeroed before it)
     unsigned long long histories, steps;
     long long q_incident, q_deposited, q_escaped;
+    unsigned long long next_history;      // work counter: next local history index to hand out
 };
 
 // Launchers (all asynchronous on `st`).
-void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, int32_t n_segs,
-                      int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q, TransportCounters* counters,
-                      int sm_count, cudaStream_t st);
+void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, const long long* seg_begin,
+                      int32_t n_segs, int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q,
+                      TransportCounters* counters, int sm_count, cudaStream_t st);
 const void* transport_kernel_symbol();
 
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,

@@ -4,17 +4,22 @@
 // CSDA loss (midpoint rule), Bohr straggling, Highland deflection without log term, 0.5 MeV cutoff deposited
 // locally, 64-bit fixed-point atomic scoring).
 //
-// Layout of the computation (B200-first, not the paper's Titan-X design):
-//  * one persistent thread per lane slot; a lane whose history ends refills itself with the next history of the
-//    launch (static stride), so warps stay full through the step loop -- the Philox counter is (step, history),
-//    never the lane, which makes any lane/history assignment give the same integers;
-//  * all arithmetic fp32 on the FP32/MUFU pipes; position is kept in voxel-local coordinates so boundary
-//    distances keep full fp32 resolution;
-//  * log2-spaced CSDA range table staged in shared memory; stopping power analytic (one MUFU.LG2 each);
-//  * deposits are converted to int64 quanta of 2^-k MeV and accumulated in a register while the history stays in
-//    one voxel; one red.global.add.u64 per voxel visit, resolved in the L2 (the int64 grid + density grid of a phase
-//    is L2-resident for the paper-shaped phantoms);
-//  * per-launch tallies (incident/deposited/escaped quanta, steps) are block-reduced, one atomic per block.
+// Layout of the computation (B200-first, not the paper's Titan-X design).  The kernel is bound by instruction
+// issue and by the XU (MUFU/conversion) pipe, never by HBM, so everything below is about instructions per step:
+//  * persistent warps; a lane whose history ends takes the next history index from a global counter (one
+//    warp-aggregated atomicAdd), so all lanes stay busy until the launch runs out of histories.  The Philox counter
+//    is (step, history), never the lane, so any lane/history assignment gives the same integers;
+//  * the step loop is warp-uniform (refill phase, then one predicated step for every live lane): the warp
+//    reconverges every iteration;
+//  * S(E), 2 % of the CSDA range, the Bohr variance and the Highland theta0^2 come from ONE float4 table in shared
+//    memory, indexed by integer operations on the bit pattern of E (no logarithm), linear in E inside an interval;
+//  * one reciprocal per step for the voxel-face distance (the nearest face is found by cross-multiplication),
+//    1/density cached per voxel visit, Gaussian factors folded under one square root each, small-angle polynomial
+//    for the polar deflection, uniform floats built with bit operations: 9 MUFU per step instead of ~27;
+//  * Philox round keys are kernel parameters (constant bank operands);
+//  * position is voxel-local (0 <= p <= h) so face distances keep full fp32 resolution;
+//  * deposits are converted to int64 quanta of 2^-k MeV and summed in a register while the history stays in one
+//    voxel; one red.global.add.u64 per voxel visit, resolved in the L2.
 #include "internal.h"
 #include "physics_tables.h"
 
@@ -25,90 +30,83 @@ namespace pbs4d {
 namespace {
 
 constexpr int   kThreads   = 128;
-constexpr float kInvMp     = 1.0f / 938.27208816f;
-constexpr float kMp        = 938.27208816f;
-constexpr float kMe        = 0.51099895f;
-constexpr float kRatio     = 0.51099895f / 938.27208816f;          // me / Mp
-constexpr float kKZA       = 0.307075f * (10.0f / 18.01528f);        // K Z/A, MeV cm2/g
-constexpr float kLogArg    = 2.0f * 0.51099895f / 75.0e-6f;          // 2 me c2 / I
-constexpr float kInvX0     = 1.0f / 36.08f;
-constexpr float kEs        = 13.6f;
 constexpr float kEcut      = 0.5f;
 constexpr float kSmax      = 1.0f;
-constexpr float kFrac      = 0.02f;
 constexpr float kTie       = 1.0f + 1.0f / 1024.0f;                  // boundary/step-limit tie tolerance (DESIGN A22)
-constexpr float kLn2       = 0.6931471805599453f;
 constexpr float kTwoPi     = 6.283185307179586f;
-constexpr float kU01       = 1.0f / 8388608.0f;
+constexpr float kPi        = 3.14159265358979f;
+constexpr float kNeg2Ln2   = -1.3862943611198906f;                  // -2 ln 2
+constexpr float kHuge      = 1.0e30f;
 
 struct Params {
     pbs4d_grid g;
     const float* __restrict__ rho;
     const DevSegment* __restrict__ segs;
-    const float* __restrict__ range_tab;      // kRangeNodes log2(R_w[g/cm2]) values
+    const long long* __restrict__ seg_begin;  // [n_segs] local index of each segment's first history (ascending)
+    const float4* __restrict__ tab;           // kTabNodes physics nodes
     int32_t n_segs;
     long long n_hist;
-    uint32_t seed_lo, seed_hi, flags;
+    uint32_t flags;
+    uint32_t k0[10], k1[10];                  // Philox round keys
     unsigned long long* Q;
     TransportCounters* counters;
 };
 
-// ---- Philox4x32-10, counter = (block, 0, g_lo, g_hi), key = seed ----
-__device__ __forceinline__ void philox(uint32_t block, uint32_t g_lo, uint32_t g_hi, uint32_t k0, uint32_t k1,
+// ---- Philox4x32-10, counter = (block, 0, g_lo, g_hi) ----
+__device__ __forceinline__ void philox(const Params& P, uint32_t block, uint32_t g_lo, uint32_t g_hi,
                                        uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3)
 {
     uint32_t c0 = block, c1 = 0u, c2 = g_lo, c3 = g_hi;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const unsigned long long pa = (unsigned long long)0xD2511F53u * c0;
-        const unsigned long long pb = (unsigned long long)0xCD9E8D57u * c2;
-        const uint32_t n0 = (uint32_t)(pb >> 32) ^ c1 ^ k0;
-        const uint32_t n2 = (uint32_t)(pa >> 32) ^ c3 ^ k1;
-        c1 = (uint32_t)pb; c3 = (uint32_t)pa; c0 = n0; c2 = n2;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ P.k0[r];
+        c2 = h0 ^ c3 ^ P.k1[r];
+        c1 = l1; c3 = l0;
     }
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
-__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * kU01; }
-
-// kinematics at kinetic energy E: a = beta^2 gamma^2 = tau (tau + 2), gam = gamma
-struct Kin { float a, gam, inv_beta2, x; };
-__device__ __forceinline__ Kin kinematics(float E)
+// u = ((x >> 9) + 0.5) 2^-23, built without an integer->float conversion: (1 + m 2^-23) - 1 + 2^-24, all exact
+__device__ __forceinline__ float u01(uint32_t x)
 {
-    Kin k;
-    const float tau = E * kInvMp;
-    k.a   = tau * (tau + 2.0f);
-    k.gam = 1.0f + tau;
-    k.inv_beta2 = __fdividef(k.gam * k.gam, k.a);
-    k.x   = 2.0f * kRatio * k.gam + kRatio * kRatio;                 // T_max = 2 me a / (1 + x)
-    return k;
+    return (__uint_as_float(0x3F800000u | (x >> 9)) - 1.0f) + 5.9604644775390625e-8f;
 }
 
-// Bethe mass stopping power of water [MeV cm2/g]:
-//   K Z/A / beta2 [ 1/2 ln(2 me a Tmax / I^2) - beta2 ] with 1/2 ln(..) = ln(2 me a / I) - 1/2 ln(1 + x)
-__device__ __forceinline__ float bethe(const Kin& k)
+__device__ __forceinline__ float fast_sqrt(float x)
 {
-    const float l1  = __log2f(kLogArg * k.a) * kLn2;
-    const float l2  = 0.5f * k.x * (1.0f - 0.5f * k.x);              // 1/2 ln(1+x), x ~ 1e-3
-    const float b2  = __fdividef(1.0f, k.inv_beta2);
-    return kKZA * k.inv_beta2 * (l1 - l2 - b2);
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float fast_rcp(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
-// CSDA range in water [g/cm2] from the shared-memory table (log2-log2 linear interpolation)
-__device__ __forceinline__ float range_water(float E, const float* tab)
+// cos(2 pi u), sin(2 pi u) for u in (0,1): the MUFU argument is moved to (-pi, pi), where sin/cos.approx are
+// accurate to ~2^-21 absolute; cos(x + pi) = -cos x
+__device__ __forceinline__ void sincos_2pi(float u, float& s, float& c)
 {
-    float x = (__log2f(E) - kRangeLog2E0) * kRangeInvStep;
-    x = fminf(fmaxf(x, 0.0f), (float)(kRangeNodes - 1) - 0.001f);
-    const int   i = (int)x;
-    const float f = x - (float)i;
-    const float a = tab[i], b = tab[i + 1];
-    return exp2f(a + f * (b - a));
+    const float a = fmaf(u, kTwoPi, -kPi);
+    s = -__sinf(a); c = -__cosf(a);
 }
 
-}  // namespace
-
-namespace {
+// table interval and fraction of an energy (integer operations on the bit pattern; see physics_tables.h)
+struct Lookup { int i; float f; };
+__device__ __forceinline__ Lookup locate(float E)
+{
+    const uint32_t b = __float_as_uint(E);
+    Lookup L;
+    L.i = min(max((int)(b >> 16) - (int)(kTabBits0 >> 16), 0), kTabNodes - 2);
+    const float e_node = __uint_as_float(b & 0xFFFF0000u);
+    const float inv_w  = __uint_as_float(0x82800000u - (b & 0x7F800000u));          // 2^(7 - exponent)
+    L.f = (E - e_node) * inv_w;
+    return L;
+}
 
 // Per-lane history state.  Position p* is voxel-local: 0 <= p <= h on each axis.
 struct Lane {
@@ -116,20 +114,19 @@ struct Lane {
     double wq_d;
     int ix, iy, iz;
     uint32_t g_lo, g_hi, m;
-    long long vox;                             // linear voxel index of the pending deposit
+    int vox;                                   // linear voxel index of the pending deposit (< 2^31 voxels)
     long long pend;                            // quanta deposited in vox and not yet flushed
-    float dens;
+    float dens, inv_dens;
 };
 
 // T3: sample history j of the launch.  Returns false if the ray misses the grid (all energy escapes).
-__device__ __forceinline__ bool start_history(const Params& P, long long j, Lane& L, long long& q_inc,
-                                              long long& q_esc)
+__device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L, long long& q_inc, long long& q_esc)
 {
-    // segment lookup: last segment with local_begin <= j
+    // segment lookup: last segment with seg_begin <= j
     int lo = 0, hi = P.n_segs - 1;
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if (P.segs[mid].local_begin <= j) lo = mid; else hi = mid - 1;
+        if (__ldg(P.seg_begin + mid) <= j) lo = mid; else hi = mid - 1;
     }
     const DevSegment& S = P.segs[lo];
     const unsigned long long g = (unsigned long long)(S.first_history + (j - S.local_begin));
@@ -137,12 +134,13 @@ __device__ __forceinline__ bool start_history(const Params& P, long long j, Lane
     L.wq = S.weight_scaled; L.wq_d = S.weight_scaled_d;
 
     uint32_t r0, r1, r2, r3;
-    philox(0u, L.g_lo, L.g_hi, P.seed_lo, P.seed_hi, r0, r1, r2, r3);
-    const float rad = sqrtf(-2.0f * logf(u01(r0)));
-    float sn, cs;
-    sincospif(2.0f * u01(r1), &sn, &cs);
+    philox(P, 0u, L.g_lo, L.g_hi, r0, r1, r2, r3);
+    const float rad = fast_sqrt(kNeg2Ln2 * __log2f(u01(r0)));
+    float sn, cs, snE, csE;
+    sincos_2pi(u01(r1), sn, cs);
+    sincos_2pi(u01(r3), snE, csE);
     float gx = rad * cs, gy = rad * sn;
-    float gE = sqrtf(-2.0f * logf(u01(r2))) * cospif(2.0f * u01(r3));
+    float gE = fast_sqrt(kNeg2Ln2 * __log2f(u01(r2))) * csE;
     if (P.flags & PBS4D_NO_SPOTSIZE) { gx = 0.0f; gy = 0.0f; }
     if (P.flags & PBS4D_NO_ESPREAD)  gE = 0.0f;
     L.E = S.energy_mev * (1.0f + 0.01f * gE);
@@ -183,130 +181,159 @@ __device__ __forceinline__ bool start_history(const Params& P, long long j, Lane
     L.px = pl[0]; L.py = pl[1]; L.pz = pl[2];
     L.dx = d[0];  L.dy = d[1];  L.dz = d[2];
     L.ix = idx[0]; L.iy = idx[1]; L.iz = idx[2];
-    L.vox = ((long long)L.iz * P.g.ny + L.iy) * P.g.nx + L.ix;
+    L.vox = (L.iz * P.g.ny + L.iy) * P.g.nx + L.ix;
     L.pend = 0;
     L.dens = __ldg(P.rho + L.vox);
+    L.inv_dens = fast_rcp(L.dens);
     return true;
 }
 
-__device__ __forceinline__ void flush(const Params& P, Lane& L)
+__device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep)
 {
     if (L.pend != 0) {
         atomicAdd(P.Q + L.vox, (unsigned long long)L.pend);
+        q_dep += L.pend;
         L.pend = 0;
     }
 }
 
 __global__ void __launch_bounds__(kThreads)
-transport_kernel(const Params P)
+transport_kernel(const __grid_constant__ Params P)
 {
-    __shared__ float s_range[kRangeNodes];
+    __shared__ float4 s_tab[kTabNodes];
     __shared__ long long s_tally[5];
-    for (int i = threadIdx.x; i < kRangeNodes; i += kThreads) s_range[i] = P.range_tab[i];
+    for (int i = threadIdx.x; i < kTabNodes; i += kThreads) s_tab[i] = P.tab[i];
     if (threadIdx.x < 5) s_tally[threadIdx.x] = 0;
     __syncthreads();
 
-    const long long stride = (long long)gridDim.x * kThreads;
-    long long next = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const unsigned lane = threadIdx.x & 31u;
     long long q_inc = 0, q_dep = 0, q_esc = 0;
-    unsigned long long n_steps = 0, n_hist = 0;
+    uint32_t n_steps = 0, n_hist = 0;
     const float hx = P.g.hx, hy = P.g.hy, hz = P.g.hz;
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
     const bool do_mcs = !(P.flags & PBS4D_NO_MCS), do_strag = !(P.flags & PBS4D_NO_STRAGGLE);
 
     Lane L;
-    bool alive = false;
+    bool alive = false, exhausted = false;
     for (;;) {
-        if (!alive) {
-            // refill this lane with its next history (T3); a lane with none left leaves the loop
-            if (next >= P.n_hist) break;
-            alive = start_history(P, next, L, q_inc, q_esc);
-            next += stride;
-            n_hist += 1;
-            if (!alive) continue;
-        }
-        // ---------------- one condensed-history step (T5-T10) ----------------
-        L.m += 1u;
-        const float dens = L.dens;
-        const Kin   k0 = kinematics(L.E);
-        const float S0 = bethe(k0);
-        const float R  = __fdividef(10.0f * range_water(L.E, s_range), dens);           // mm, local medium
-
-        // T6: distance to the voxel faces (voxel-local coordinates)
-        const float idx_ = __frcp_rn(L.dx), idy_ = __frcp_rn(L.dy), idz_ = __frcp_rn(L.dz);
-        float sax = L.dx > 0.0f ? (hx - L.px) * idx_ : (L.dx < 0.0f ? -L.px * idx_ : INFINITY);
-        float say = L.dy > 0.0f ? (hy - L.py) * idy_ : (L.dy < 0.0f ? -L.py * idy_ : INFINITY);
-        float saz = L.dz > 0.0f ? (hz - L.pz) * idz_ : (L.dz < 0.0f ? -L.pz * idz_ : INFINITY);
-        sax = fmaxf(sax, 0.0f); say = fmaxf(say, 0.0f); saz = fmaxf(saz, 0.0f);
-        const float s_b   = fminf(sax, fminf(say, saz));
-        const float s_lim = fminf(kSmax, kFrac * R);
-        const bool  crossing = s_b <= s_lim * kTie;
-        const float s = crossing ? s_b : s_lim;
-
-        // T7: midpoint-rule mean loss
-        const float t   = dens * s * 0.1f;                                               // g/cm2
-        const float Em  = fmaxf(L.E - 0.5f * S0 * t, 1.0e-3f);
-        const Kin   km  = kinematics(Em);
-        const float dEm = bethe(km) * t;
-
-        // T8: straggling (Philox block m)
-        uint32_t r0, r1, r2, r3;
-        philox(L.m, L.g_lo, L.g_hi, P.seed_lo, P.seed_hi, r0, r1, r2, r3);
-        float dE = dEm;
-        if (do_strag) {
-            const float tmax = __fdividef(2.0f * kMe * km.a, 1.0f + km.x);
-            const float b2   = __fdividef(1.0f, km.inv_beta2);
-            const float var  = 0.5f * kKZA * km.inv_beta2 * tmax * (1.0f - 0.5f * b2) * t;
-            const float gg   = sqrtf(-2.0f * logf(u01(r2))) * cospif(2.0f * u01(r3));
-            dE = dEm + sqrtf(var) * gg;
-        }
-        dE = fminf(fmaxf(dE, 0.0f), L.E);
-        if (L.E - dE <= kEcut) { dE = L.E; alive = false; }
-
-        // T9/T11: score into the voxel the step lay in (register accumulation, flushed on voxel change)
-        const long long q = __float2ll_rn(dE * L.wq);
-        L.pend += q; q_dep += q; n_steps += 1;
-
-        L.px += s * L.dx; L.py += s * L.dy; L.pz += s * L.dz;
-
-        // T10: boundary-limited step -> snap every axis attaining the minimum onto its face
-        bool moved = false;
-        if (crossing) {
-            if (sax == s_b) { if (L.dx > 0.0f) { L.ix += 1; L.px = 0.0f; } else { L.ix -= 1; L.px = hx; } moved = true; }
-            if (say == s_b) { if (L.dy > 0.0f) { L.iy += 1; L.py = 0.0f; } else { L.iy -= 1; L.py = hy; } moved = true; }
-            if (saz == s_b) { if (L.dz > 0.0f) { L.iz += 1; L.pz = 0.0f; } else { L.iz -= 1; L.pz = hz; } moved = true; }
-        }
-
-        // T9: Highland deflection at the end of the step (kinematics at Em), branch-free orthonormal basis
-        if (do_mcs) {
-            const float pv  = kMp * __fdividef(km.a, km.gam);
-            const float th0 = __fdividef(kEs, pv) * sqrtf(t * kInvX0);
-            const float th  = th0 * sqrtf(-2.0f * logf(u01(r0)));
-            float sp, cp, st, ct;
-            sincospif(2.0f * u01(r1), &sp, &cp);
-            sincosf(th, &st, &ct);
-            const float sw = copysignf(1.0f, L.dz);
-            const float aa = -__frcp_rn(sw + L.dz);
-            const float bb = L.dx * L.dy * aa;
-            const float e1x = 1.0f + sw * L.dx * L.dx * aa, e1y = sw * bb, e1z = -sw * L.dx;
-            const float e2x = bb, e2y = sw + L.dy * L.dy * aa, e2z = -L.dy;
-            const float ux = cp * e1x + sp * e2x, uy = cp * e1y + sp * e2y, uz = cp * e1z + sp * e2z;
-            const float nxd = ct * L.dx + st * ux, nyd = ct * L.dy + st * uy, nzd = ct * L.dz + st * uz;
-            const float inv = rsqrtf(nxd * nxd + nyd * nyd + nzd * nzd);
-            L.dx = nxd * inv; L.dy = nyd * inv; L.dz = nzd * inv;
-        }
-        L.E -= dE;
-
-        if (!alive) { flush(P, L); continue; }
-        if (moved) {
-            flush(P, L);
-            if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
-                q_esc += __double2ll_rn((double)L.E * L.wq_d);                           // left the grid
-                alive = false;
-                continue;
+        // ---------------- refill phase: dead lanes take the next history indices of the launch ----------------
+        const unsigned want = __ballot_sync(0xffffffffu, !alive && !exhausted);
+        if (want) {
+            const int leader = __ffs(want) - 1;
+            unsigned long long base = 0;
+            if (lane == (unsigned)leader) base = atomicAdd(&P.counters->next_history, (unsigned long long)__popc(want));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (!alive && !exhausted) {
+                const long long j = (long long)base + __popc(want & ((1u << lane) - 1u));
+                if (j < P.n_hist) {
+                    Lane T;                                   // the out-of-line call writes a stack temporary;
+                    long long qi = 0, qe = 0;                 // the loop's own state stays in registers
+                    alive = start_history(P, j, T, qi, qe);
+                    L = T; q_inc += qi; q_esc += qe; n_hist += 1;
+                }
+                else exhausted = true;
             }
-            L.vox  = ((long long)L.iz * ny + L.iy) * nx + L.ix;
-            L.dens = __ldg(P.rho + L.vox);
+        }
+        if (!__any_sync(0xffffffffu, alive)) {
+            if (__all_sync(0xffffffffu, exhausted)) break;
+            continue;
+        }
+        if (alive) {
+            // ---------------- one condensed-history step (T5-T10) ----------------
+            L.m += 1u;
+            const float dens = L.dens;
+            const Lookup k0 = locate(L.E);
+            const float4 A0 = s_tab[k0.i], B0 = s_tab[k0.i + 1];
+            const float rs = fmaf(k0.f, B0.x - A0.x, A0.x);                  // 0.2 R_w(E)
+            const float S0 = fmaf(k0.f, B0.y - A0.y, A0.y);
+            const float s_lim = fminf(kSmax, rs * L.inv_dens);
+
+            // T6: nearest voxel face.  Per axis: numerator = distance to the face ahead, denominator = |d|;
+            // the smallest quotient is found by cross-multiplication, then one reciprocal.
+            float numx = L.dx > 0.0f ? hx - L.px : L.px, denx = fabsf(L.dx);
+            float numy = L.dy > 0.0f ? hy - L.py : L.py, deny = fabsf(L.dy);
+            float numz = L.dz > 0.0f ? hz - L.pz : L.pz, denz = fabsf(L.dz);
+            numx = fmaxf(numx, 0.0f); numy = fmaxf(numy, 0.0f); numz = fmaxf(numz, 0.0f);
+            if (denx == 0.0f) { numx = kHuge; denx = 1.0f; }
+            if (deny == 0.0f) { numy = kHuge; deny = 1.0f; }
+            if (denz == 0.0f) { numz = kHuge; denz = 1.0f; }
+            float num = numz, den = denz;                                    // z first: the usual beam axis wins ties
+            if (numx * den < num * denx) { num = numx; den = denx; }
+            if (numy * den < num * deny) { num = numy; den = deny; }
+            const float s_b = num * fast_rcp(den);
+            const bool  crossing = s_b <= s_lim * kTie;
+            const float s = crossing ? s_b : s_lim;
+
+            // T7: midpoint-rule mean loss
+            const float t   = dens * s * 0.1f;                                // g/cm2
+            const float Em  = fmaxf(L.E - 0.5f * S0 * t, 0.25f);
+            const Lookup km = locate(Em);
+            const float4 Am = s_tab[km.i], Bm = s_tab[km.i + 1];
+            const float Sm  = fmaf(km.f, Bm.y - Am.y, Am.y);
+            const float dEm = Sm * t;
+
+            // T8: straggling (Philox block m): sigma g = sqrt(V t (-2 ln u2)) cos(2 pi u3)
+            uint32_t r0, r1, r2, r3;
+            philox(P, L.m, L.g_lo, L.g_hi, r0, r1, r2, r3);
+            float dE = dEm;
+            if (do_strag) {
+                const float V2 = fmaf(km.f, Bm.z - Am.z, Am.z);
+                const float a3 = fmaf(u01(r3), kTwoPi, -kPi);
+                dE = fmaf(fast_sqrt(-V2 * t * __log2f(u01(r2))), -__cosf(a3), dEm);
+            }
+            dE = fminf(fmaxf(dE, 0.0f), L.E);
+            if (L.E - dE <= kEcut) { dE = L.E; alive = false; }
+
+            // T9/T11: score into the voxel the step lay in (register accumulation, flushed on voxel change)
+            L.pend += __float2ll_rn(dE * L.wq);
+            n_steps += 1;
+
+            L.px = fmaf(s, L.dx, L.px); L.py = fmaf(s, L.dy, L.py); L.pz = fmaf(s, L.dz, L.pz);
+
+            // T10: boundary-limited step -> snap every axis attaining the minimum onto its face
+            bool moved = false;
+            if (crossing) {
+                if (numx * den == num * denx) { if (L.dx > 0.0f) { L.ix += 1; L.px = 0.0f; } else { L.ix -= 1; L.px = hx; } moved = true; }
+                if (numy * den == num * deny) { if (L.dy > 0.0f) { L.iy += 1; L.py = 0.0f; } else { L.iy -= 1; L.py = hy; } moved = true; }
+                if (numz * den == num * denz) { if (L.dz > 0.0f) { L.iz += 1; L.pz = 0.0f; } else { L.iz -= 1; L.pz = hz; } moved = true; }
+            }
+
+            // T9: Highland deflection at the end of the step (kinematics at Em), branch-free orthonormal basis;
+            // theta^2 = T t (-2 ln u0); sin and cos of the (small) polar angle by their Taylor polynomials
+            if (do_mcs) {
+                const float T2  = fmaf(km.f, Bm.w - Am.w, Am.w);
+                const float th2 = -T2 * t * __log2f(u01(r0));
+                const float th  = fast_sqrt(th2);
+                const float st  = th * fmaf(th2, fmaf(th2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+                const float ct  = fmaf(th2, fmaf(th2, fmaf(th2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
+                float sp, cp;
+                sincos_2pi(u01(r1), sp, cp);
+                const float sw = copysignf(1.0f, L.dz);
+                const float aa = -fast_rcp(sw + L.dz);
+                const float bb = L.dx * L.dy * aa;
+                const float e1x = fmaf(sw * L.dx, L.dx * aa, 1.0f), e1y = sw * bb, e1z = -sw * L.dx;
+                const float e2x = bb, e2y = fmaf(L.dy, L.dy * aa, sw), e2z = -L.dy;
+                const float ux = fmaf(cp, e1x, sp * e2x), uy = fmaf(cp, e1y, sp * e2y), uz = fmaf(cp, e1z, sp * e2z);
+                const float nxd = fmaf(ct, L.dx, st * ux), nyd = fmaf(ct, L.dy, st * uy), nzd = fmaf(ct, L.dz, st * uz);
+                const float n2  = fmaf(nxd, nxd, fmaf(nyd, nyd, nzd * nzd));
+                const float inv = fmaf(-0.5f, n2, 1.5f);                      // 1/sqrt(n2) to first order, n2 = 1 + O(1e-6)
+                L.dx = nxd * inv; L.dy = nyd * inv; L.dz = nzd * inv;
+            }
+            L.E -= dE;
+
+            if (!alive) {
+                flush(P, L, q_dep);
+            } else if (moved) {
+                flush(P, L, q_dep);
+                if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
+                    q_esc += __double2ll_rn((double)L.E * L.wq_d);                           // left the grid
+                    alive = false;
+                } else {
+                    L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
+                    L.dens = __ldg(P.rho + L.vox);
+                    L.inv_dens = fast_rcp(L.dens);
+                }
+            }
         }
     }
 
@@ -317,7 +344,7 @@ transport_kernel(const Params P)
         long long x = v[c];
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
-        if ((threadIdx.x & 31) == 0) atomicAdd((unsigned long long*)&s_tally[c], (unsigned long long)x);
+        if (lane == 0) atomicAdd((unsigned long long*)&s_tally[c], (unsigned long long)x);
     }
     __syncthreads();
     if (threadIdx.x < 5) {
@@ -334,25 +361,31 @@ transport_kernel(const Params P)
 
 const void* transport_kernel_symbol() { return (const void*)transport_kernel; }
 
-static float* g_range_tab_dev[16] = { nullptr };   // one table per device, built on first use
+static float4* g_tab_dev[16] = { nullptr };   // one table per device, built on first use
 
-void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, int32_t n_segs,
-                      int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q, TransportCounters* counters,
-                      int sm_count, cudaStream_t st)
+void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, const long long* seg_begin,
+                      int32_t n_segs, int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q,
+                      TransportCounters* counters, int sm_count, cudaStream_t st)
 {
     int dev = 0;
     cudaGetDevice(&dev);
-    if (dev >= 0 && dev < 16 && !g_range_tab_dev[dev]) {
-        float host_tab[kRangeNodes];
-        build_range_table(host_tab);
-        cudaMalloc(&g_range_tab_dev[dev], sizeof(host_tab));
-        cudaMemcpy(g_range_tab_dev[dev], host_tab, sizeof(host_tab), cudaMemcpyHostToDevice);
+    if (dev >= 0 && dev < 16 && !g_tab_dev[dev]) {
+        static TabNode host_tab[kTabNodes];
+        build_physics_table(host_tab);
+        cudaMalloc(&g_tab_dev[dev], sizeof(host_tab));
+        cudaMemcpy(g_tab_dev[dev], host_tab, sizeof(host_tab), cudaMemcpyHostToDevice);
     }
     Params P;
-    P.g = g; P.rho = rho; P.segs = segs; P.range_tab = g_range_tab_dev[dev];
-    P.n_segs = n_segs; P.n_hist = n_hist;
-    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32); P.flags = flags;
+    P.g = g; P.rho = rho; P.segs = segs; P.seg_begin = seg_begin; P.tab = g_tab_dev[dev];
+    P.n_segs = n_segs; P.n_hist = n_hist; P.flags = flags;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
     P.Q = (unsigned long long*)Q; P.counters = counters;
+    static bool configured = false;
+    if (!configured) {        // 22.5 KB table per CTA: ask for a shared-memory carve-out that keeps all CTAs resident
+        cudaFuncSetAttribute(transport_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+        configured = true;
+    }
     int per_sm = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, transport_kernel, kThreads, 0);
     if (per_sm < 1) per_sm = 1;
