@@ -109,13 +109,16 @@ bool grid_ok(const pbs4d_grid* g)
 
 void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
 {
+    // device buffers are kept across calls (DevBuf::ensure reuses an allocation that is large enough): a plan that
+    // is recomputed on the same grids costs no cudaMalloc/cudaFree
     ctx->n_phases = n_phases; ctx->dose_grid = g;
-    ctx->rho.clear(); ctx->q.clear(); ctx->dose.clear(); ctx->accE.clear(); ctx->accM.clear(); ctx->dvf.clear();
-    for (int p = 0; p < n_phases; ++p) {
-        ctx->rho.emplace_back(new DevBuf); ctx->q.emplace_back(new DevBuf); ctx->dose.emplace_back(new DevBuf);
-        ctx->accE.emplace_back(new DevBuf); ctx->accM.emplace_back(new DevBuf);
-    }
+    auto fit = [&](std::vector<std::unique_ptr<DevBuf>>& v) {
+        v.resize(n_phases);
+        for (auto& b : v) if (!b) b.reset(new DevBuf);
+    };
+    fit(ctx->rho); fit(ctx->q); fit(ctx->dose); fit(ctx->accE); fit(ctx->accM);
     ctx->dvf.resize(n_phases);
+    for (auto& d : ctx->dvf) { d.set = false; d.ref = -1; }
     ctx->have_dose.assign(n_phases, false);
     ctx->have_acc.assign(n_phases, false);
     ctx->have_density = false;
