@@ -80,6 +80,12 @@ __device__ __forceinline__ float fast_sqrt(float x)
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float fast_log2(float x)       // x >= 2^-24 here: no denormal pre-scaling needed
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float fast_rcp(float x)
 {
     float y;
@@ -135,12 +141,12 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
 
     uint32_t r0, r1, r2, r3;
     philox(P, 0u, L.g_lo, L.g_hi, r0, r1, r2, r3);
-    const float rad = fast_sqrt(kNeg2Ln2 * __log2f(u01(r0)));
+    const float rad = fast_sqrt(kNeg2Ln2 * fast_log2(u01(r0)));
     float sn, cs, snE, csE;
     sincos_2pi(u01(r1), sn, cs);
     sincos_2pi(u01(r3), snE, csE);
     float gx = rad * cs, gy = rad * sn;
-    float gE = fast_sqrt(kNeg2Ln2 * __log2f(u01(r2))) * csE;
+    float gE = fast_sqrt(kNeg2Ln2 * fast_log2(u01(r2))) * csE;
     if (P.flags & PBS4D_NO_SPOTSIZE) { gx = 0.0f; gy = 0.0f; }
     if (P.flags & PBS4D_NO_ESPREAD)  gE = 0.0f;
     L.E = S.energy_mev * (1.0f + 0.01f * gE);
@@ -159,7 +165,8 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
     for (int k = 0; k < 3; ++k) {
         const float lo_k = o[k], hi_k = o[k] + (float)n[k] * h[k];
         if (d[k] == 0.0f) { if (r[k] < lo_k || r[k] >= hi_k) miss = true; continue; }
-        float t1 = (lo_k - r[k]) / d[k], t2 = (hi_k - r[k]) / d[k];
+        const float inv_d = fast_rcp(d[k]);
+        float t1 = (lo_k - r[k]) * inv_d, t2 = (hi_k - r[k]) * inv_d;
         if (t1 > t2) { const float tt = t1; t1 = t2; t2 = tt; }
         if (t1 > t_in) { t_in = t1; ax = k; }
         if (t2 < t_out) t_out = t2;
@@ -169,7 +176,7 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const float rk = r[k] + t_in * d[k];
-        int i = (int)floorf((rk - o[k]) / h[k]);
+        int i = (int)floorf(__fdividef(rk - o[k], h[k]));
         i = max(0, min(i, n[k] - 1));
         idx[k] = i;
         pl[k] = fminf(fmaxf(rk - (o[k] + (float)i * h[k]), 0.0f), h[k]);
@@ -190,11 +197,9 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
 
 __device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep)
 {
-    if (L.pend != 0) {
-        atomicAdd(P.Q + L.vox, (unsigned long long)L.pend);
-        q_dep += L.pend;
-        L.pend = 0;
-    }
+    atomicAdd(P.Q + L.vox, (unsigned long long)L.pend);
+    q_dep += L.pend;
+    L.pend = 0;
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -257,9 +262,16 @@ transport_kernel(const __grid_constant__ Params P)
             if (denx == 0.0f) { numx = kHuge; denx = 1.0f; }
             if (deny == 0.0f) { numy = kHuge; deny = 1.0f; }
             if (denz == 0.0f) { numz = kHuge; denz = 1.0f; }
-            float num = numz, den = denz;                                    // z first: the usual beam axis wins ties
-            if (numx * den < num * denx) { num = numx; den = denx; }
-            if (numy * den < num * deny) { num = numy; den = deny; }
+            // x against z, then y against the winner; equal cross products mark axes that attain the minimum together
+            const float cxz = numx * denz, czx = numz * denx;
+            const bool  x_lt = cxz < czx;
+            float num = x_lt ? numx : numz, den = x_lt ? denx : denz;
+            bool  mx = cxz <= czx, mz = !x_lt;
+            const float cy = numy * den, cw = num * deny;
+            const bool  y_lt = cy < cw;
+            num = y_lt ? numy : num; den = y_lt ? deny : den;
+            bool  my = cy <= cw;
+            mx = mx && !y_lt; mz = mz && !y_lt;
             const float s_b = num * fast_rcp(den);
             const bool  crossing = s_b <= s_lim * kTie;
             const float s = crossing ? s_b : s_lim;
@@ -279,7 +291,7 @@ transport_kernel(const __grid_constant__ Params P)
             if (do_strag) {
                 const float V2 = fmaf(km.f, Bm.z - Am.z, Am.z);
                 const float a3 = fmaf(u01(r3), kTwoPi, -kPi);
-                dE = fmaf(fast_sqrt(-V2 * t * __log2f(u01(r2))), -__cosf(a3), dEm);
+                dE = fmaf(fast_sqrt(-V2 * t * fast_log2(u01(r2))), -__cosf(a3), dEm);
             }
             dE = fminf(fmaxf(dE, 0.0f), L.E);
             if (L.E - dE <= kEcut) { dE = L.E; alive = false; }
@@ -290,19 +302,20 @@ transport_kernel(const __grid_constant__ Params P)
 
             L.px = fmaf(s, L.dx, L.px); L.py = fmaf(s, L.dy, L.py); L.pz = fmaf(s, L.dz, L.pz);
 
-            // T10: boundary-limited step -> snap every axis attaining the minimum onto its face
-            bool moved = false;
-            if (crossing) {
-                if (numx * den == num * denx) { if (L.dx > 0.0f) { L.ix += 1; L.px = 0.0f; } else { L.ix -= 1; L.px = hx; } moved = true; }
-                if (numy * den == num * deny) { if (L.dy > 0.0f) { L.iy += 1; L.py = 0.0f; } else { L.iy -= 1; L.py = hy; } moved = true; }
-                if (numz * den == num * denz) { if (L.dz > 0.0f) { L.iz += 1; L.pz = 0.0f; } else { L.iz -= 1; L.pz = hz; } moved = true; }
+            // T10: boundary-limited step -> snap every axis attaining the minimum onto its face (branch-free)
+            mx = mx && crossing; my = my && crossing; mz = mz && crossing;
+            {
+                const bool fx = L.dx > 0.0f, fy = L.dy > 0.0f, fz = L.dz > 0.0f;
+                L.ix += mx ? (fx ? 1 : -1) : 0; L.px = mx ? (fx ? 0.0f : hx) : L.px;
+                L.iy += my ? (fy ? 1 : -1) : 0; L.py = my ? (fy ? 0.0f : hy) : L.py;
+                L.iz += mz ? (fz ? 1 : -1) : 0; L.pz = mz ? (fz ? 0.0f : hz) : L.pz;
             }
 
             // T9: Highland deflection at the end of the step (kinematics at Em), branch-free orthonormal basis;
             // theta^2 = T t (-2 ln u0); sin and cos of the (small) polar angle by their Taylor polynomials
             if (do_mcs) {
                 const float T2  = fmaf(km.f, Bm.w - Am.w, Am.w);
-                const float th2 = -T2 * t * __log2f(u01(r0));
+                const float th2 = -T2 * t * fast_log2(u01(r0));
                 const float th  = fast_sqrt(th2);
                 const float st  = th * fmaf(th2, fmaf(th2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
                 const float ct  = fmaf(th2, fmaf(th2, fmaf(th2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
@@ -321,17 +334,17 @@ transport_kernel(const __grid_constant__ Params P)
             }
             L.E -= dE;
 
-            if (!alive) {
+            if (crossing || !alive) {
                 flush(P, L, q_dep);
-            } else if (moved) {
-                flush(P, L, q_dep);
-                if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
-                    q_esc += __double2ll_rn((double)L.E * L.wq_d);                           // left the grid
-                    alive = false;
-                } else {
-                    L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
-                    L.dens = __ldg(P.rho + L.vox);
-                    L.inv_dens = fast_rcp(L.dens);
+                if (alive) {
+                    if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
+                        q_esc += __double2ll_rn((double)L.E * L.wq_d);                       // left the grid
+                        alive = false;
+                    } else {
+                        L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
+                        L.dens = __ldg(P.rho + L.vox);
+                        L.inv_dens = fast_rcp(L.dens);
+                    }
                 }
             }
         }
