@@ -16,26 +16,30 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 namespace pbs4d {
 
 namespace {
 
-struct AxisMap { float p; int i0, i1; float w; bool ok; };
+// One axis of the subvoxel -> DVF-cell map (A2, A3): subvoxel centre p, lower DVF node i0, upper node i0 + d1,
+// weight w, and whether the centre lies inside the DVF grid's voxel extent.  It depends on (voxel index, subvoxel
+// index) of that axis only, so a CTA computes it once per axis for its tile and keeps it in shared memory.
+struct __align__(16) AxisEntry { float p, w; int i0; int flags; };      // flags: bit0 = d1, bit1 = ok
 
-// subvoxel centre on one axis and its DVF-grid cell/weight
-__device__ __forceinline__ AxisMap axis_map(float o, float h, int i, int a, int ns, float od, float hd, int nd)
+__device__ __forceinline__ AxisEntry axis_map(float o, float h, int i, int a, int ns, float od, float hd, int nd)
 {
-    AxisMap m;
+    AxisEntry m;
     const float f = __fdiv_rn(__fadd_rn((float)a, 0.5f), (float)ns);
     m.p = __fadd_rn(o, __fmul_rn(__fadd_rn((float)i, f), h));
     float g = __fsub_rn(__fdiv_rn(__fsub_rn(m.p, od), hd), 0.5f);
-    m.ok = (g >= -0.5f) && (g < __fsub_rn((float)nd, 0.5f));
+    const bool ok = (g >= -0.5f) && (g < __fsub_rn((float)nd, 0.5f));
     g = fminf(fmaxf(g, 0.0f), (float)(nd - 1));
     int k = (int)floorf(g);
     k = max(min(k, nd - 2), 0);
     m.i0 = k;
-    m.i1 = min(k + 1, nd - 1);
     m.w  = __fsub_rn(g, (float)k);
+    m.flags = (min(k + 1, nd - 1) - k) | (ok ? 2 : 0);
     return m;
 }
 
@@ -52,61 +56,91 @@ __device__ __forceinline__ bool dest_index(float q, float o, float h, int n, int
     return true;
 }
 
+// planar [3][N] displacement field -> one float4 {ux, uy, uz, 0} per DVF node, so that a trilinear corner is one
+// 128-bit load instead of three 32-bit loads
+__global__ void dvf_interleave_kernel(size_t n, const float* __restrict__ ux, const float* __restrict__ uy,
+                                      const float* __restrict__ uz, float4* __restrict__ out)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        out[i] = make_float4(ux[i], uy[i], uz[i], 0.0f);
+}
+
+constexpr int kTileX = 32, kTileY = 4;
+
 struct PushParams {
     pbs4d_grid src, dvf, ref;
     const float* __restrict__ dose;
     const float* __restrict__ rho;
-    const float* __restrict__ ux;
-    const float* __restrict__ uy;
-    const float* __restrict__ uz;
+    const float4* __restrict__ U;            // interleaved DVF
     int nsx, nsy, nsz;
     unsigned long long* E;
     unsigned long long* M;
     AccCounters* counters;
 };
 
-__global__ void __launch_bounds__(256)
-emtm_push_kernel(const PushParams P)
+__global__ void __launch_bounds__(kTileX * kTileY)
+emtm_push_kernel(const __grid_constant__ PushParams P)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    extern __shared__ AxisEntry s_map[];
+    AxisEntry* sx = s_map;                               // [nsx][32]   (subvoxel-major: conflict-free 128-bit reads)
+    AxisEntry* sy = sx + kTileX * P.nsx;                 // [4][nsy]
+    AxisEntry* sz = sy + kTileY * P.nsy;                 // [nsz]
+    const int tid = threadIdx.y * kTileX + threadIdx.x;
+    const int i = blockIdx.x * kTileX + threadIdx.x;
+    const int j = blockIdx.y * kTileY + threadIdx.y;
     const int k = blockIdx.z;
-    unsigned long long n_ref = 0, n_dvf = 0;
+    const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy;
+    for (int e = tid; e < n_x + n_y + P.nsz; e += kTileX * kTileY) {
+        if (e < n_x)
+            s_map[e] = axis_map(P.src.ox, P.src.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
+                                P.dvf.ox, P.dvf.hx, P.dvf.nx);
+        else if (e < n_x + n_y)
+            s_map[e] = axis_map(P.src.oy, P.src.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
+                                P.dvf.oy, P.dvf.hy, P.dvf.ny);
+        else
+            s_map[e] = axis_map(P.src.oz, P.src.hz, k, e - n_x - n_y, P.nsz, P.dvf.oz, P.dvf.hz, P.dvf.nz);
+    }
+    __syncthreads();
+
+    unsigned n_ref = 0, n_dvf = 0;
     if (i < P.src.nx && j < P.src.ny) {
         const size_t v = ((size_t)k * P.src.ny + j) * P.src.nx + i;
-        const float rho = P.rho[v], dose = P.dose[v];
+        const float rho = __ldg(P.rho + v), dose = __ldg(P.dose + v);
         const long long m_q = __double2ll_rn(__dmul_rn((double)rho, 16777216.0));
         const long long e_q = __double2ll_rn(__dmul_rn(__dmul_rn((double)rho, (double)dose), 4294967296.0));
-        long long run_dst = -1; long long run_cnt = 0;
+        int run_dst = -1, run_cnt = 0;
         const int dnx = P.dvf.nx, dny = P.dvf.ny;
+        const float orx = P.ref.ox, ory = P.ref.oy, orz = P.ref.oz, hrx = P.ref.hx, hry = P.ref.hy, hrz = P.ref.hz;
+        const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
         for (int c = 0; c < P.nsz; ++c) {
-            const AxisMap mz = axis_map(P.src.oz, P.src.hz, k, c, P.nsz, P.dvf.oz, P.dvf.hz, P.dvf.nz);
+            const AxisEntry mz = sz[c];
             for (int b = 0; b < P.nsy; ++b) {
-                const AxisMap my = axis_map(P.src.oy, P.src.hy, j, b, P.nsy, P.dvf.oy, P.dvf.hy, P.dvf.ny);
-                const size_t r00 = ((size_t)mz.i0 * dny + my.i0) * dnx, r01 = ((size_t)mz.i0 * dny + my.i1) * dnx;
-                const size_t r10 = ((size_t)mz.i1 * dny + my.i0) * dnx, r11 = ((size_t)mz.i1 * dny + my.i1) * dnx;
+                const AxisEntry my = sy[threadIdx.y * P.nsy + b];
+                const int r00 = (mz.i0 * dny + my.i0) * dnx;
+                const int r01 = r00 + (my.flags & 1) * dnx;
+                const int r10 = r00 + (mz.flags & 1) * dny * dnx;
+                const int r11 = r10 + (my.flags & 1) * dnx;
+                const bool ok_zy = (mz.flags & my.flags & 2) != 0;
                 for (int a = 0; a < P.nsx; ++a) {
-                    const AxisMap mx = axis_map(P.src.ox, P.src.hx, i, a, P.nsx, P.dvf.ox, P.dvf.hx, P.dvf.nx);
-                    if (!(mx.ok && my.ok && mz.ok)) { n_dvf += 1; continue; }
-                    float q[3];
-                    const float* comp[3] = { P.ux, P.uy, P.uz };
-                    const float  pc[3]   = { mx.p, my.p, mz.p };
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        const float* u = comp[d];
-                        const float c00 = lerp_rn(__ldg(u + r00 + mx.i0), __ldg(u + r00 + mx.i1), mx.w);
-                        const float c01 = lerp_rn(__ldg(u + r01 + mx.i0), __ldg(u + r01 + mx.i1), mx.w);
-                        const float c10 = lerp_rn(__ldg(u + r10 + mx.i0), __ldg(u + r10 + mx.i1), mx.w);
-                        const float c11 = lerp_rn(__ldg(u + r11 + mx.i0), __ldg(u + r11 + mx.i1), mx.w);
-                        const float c0  = lerp_rn(c00, c01, my.w);
-                        const float c1  = lerp_rn(c10, c11, my.w);
-                        q[d] = __fadd_rn(pc[d], lerp_rn(c0, c1, mz.w));
-                    }
+                    const AxisEntry mx = sx[a * kTileX + threadIdx.x];
+                    if (!(ok_zy && (mx.flags & 2))) { n_dvf += 1; continue; }
+                    const int x0 = mx.i0, x1 = mx.i0 + (mx.flags & 1);
+                    const float4 a000 = __ldg(P.U + r00 + x0), a001 = __ldg(P.U + r00 + x1);
+                    const float4 a010 = __ldg(P.U + r01 + x0), a011 = __ldg(P.U + r01 + x1);
+                    const float4 a100 = __ldg(P.U + r10 + x0), a101 = __ldg(P.U + r10 + x1);
+                    const float4 a110 = __ldg(P.U + r11 + x0), a111 = __ldg(P.U + r11 + x1);
+                    // per component: 4 lerps in x, 2 in y, 1 in z (A3), then q = p + u (A4)
+#define PBS4D_TRILERP(cmp) lerp_rn(lerp_rn(lerp_rn(a000.cmp, a001.cmp, mx.w), lerp_rn(a010.cmp, a011.cmp, mx.w), my.w), \
+                                   lerp_rn(lerp_rn(a100.cmp, a101.cmp, mx.w), lerp_rn(a110.cmp, a111.cmp, mx.w), my.w), mz.w)
+                    const float qx = __fadd_rn(mx.p, PBS4D_TRILERP(x));
+                    const float qy = __fadd_rn(my.p, PBS4D_TRILERP(y));
+                    const float qz = __fadd_rn(mz.p, PBS4D_TRILERP(z));
+#undef PBS4D_TRILERP
                     int ix, iy, iz;
-                    if (!dest_index(q[0], P.ref.ox, P.ref.hx, P.ref.nx, ix) ||
-                        !dest_index(q[1], P.ref.oy, P.ref.hy, P.ref.ny, iy) ||
-                        !dest_index(q[2], P.ref.oz, P.ref.hz, P.ref.nz, iz)) { n_ref += 1; continue; }
-                    const long long dst = ((long long)iz * P.ref.ny + iy) * P.ref.nx + ix;
+                    if (!dest_index(qx, orx, hrx, rnx, ix) || !dest_index(qy, ory, hry, rny, iy) ||
+                        !dest_index(qz, orz, hrz, rnz, iz)) { n_ref += 1; continue; }
+                    const int dst = (iz * rny + iy) * rnx + ix;
                     if (dst == run_dst) { run_cnt += 1; continue; }
                     if (run_cnt) {
                         atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
@@ -127,77 +161,133 @@ emtm_push_kernel(const PushParams P)
         n_ref += __shfl_xor_sync(0xffffffffu, n_ref, off);
         n_dvf += __shfl_xor_sync(0xffffffffu, n_dvf, off);
     }
-    if (((threadIdx.y * blockDim.x + threadIdx.x) & 31) == 0) {
-        if (n_ref) atomicAdd(&P.counters->dropped_ref, n_ref);
-        if (n_dvf) atomicAdd(&P.counters->dropped_dvf, n_dvf);
+    if (threadIdx.x == 0) {
+        if (n_ref) atomicAdd(&P.counters->dropped_ref, (unsigned long long)n_ref);
+        if (n_dvf) atomicAdd(&P.counters->dropped_dvf, (unsigned long long)n_dvf);
     }
 }
 
 constexpr int kMaxSrc = 32;
+struct CoverParams { pbs4d_grid ref; int n_src; pbs4d_grid dvf[kMaxSrc]; unsigned char* flags; };
+
+// mask (A6): a reference voxel is kept iff its centre lies inside the voxel extent of every source
+// DVF.  The test is separable, so it is evaluated once per axis index into flags[nx | ny | nz] (1 = covered).
+__global__ void emtm_cover_kernel(const __grid_constant__ CoverParams P)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nx = P.ref.nx, ny = P.ref.ny, nz = P.ref.nz;
+    if (e >= nx + ny + nz) return;
+    const int axis = e < nx ? 0 : (e < nx + ny ? 1 : 2);
+    const int i = axis == 0 ? e : (axis == 1 ? e - nx : e - nx - ny);
+    const float o = axis == 0 ? P.ref.ox : (axis == 1 ? P.ref.oy : P.ref.oz);
+    const float h = axis == 0 ? P.ref.hx : (axis == 1 ? P.ref.hy : P.ref.hz);
+    const float p = __fadd_rn(o, __fmul_rn(__fadd_rn((float)i, 0.5f), h));
+    bool covered = true;
+    for (int s = 0; s < P.n_src; ++s) {
+        const pbs4d_grid& d = P.dvf[s];
+        const float od = axis == 0 ? d.ox : (axis == 1 ? d.oy : d.oz);
+        const float hd = axis == 0 ? d.hx : (axis == 1 ? d.hy : d.hz);
+        const int   nd = axis == 0 ? d.nx : (axis == 1 ? d.ny : d.nz);
+        const float g = __fsub_rn(__fdiv_rn(__fsub_rn(p, od), hd), 0.5f);
+        covered = covered && (g >= -0.5f) && (g < __fsub_rn((float)nd, 0.5f));
+    }
+    P.flags[e] = covered ? 1 : 0;
+}
+
 struct FinalizeParams {
     pbs4d_grid ref;
     const float* __restrict__ dose_ref;
     int n_src;
     const long long* E[kMaxSrc];
     const long long* M[kMaxSrc];
-    pbs4d_grid dvf[kMaxSrc];
+    const unsigned char* __restrict__ flags;
     float* out;
 };
 
-__device__ __forceinline__ bool covered_axis(float o, float h, int i, float od, float hd, int nd)
+__device__ __forceinline__ double ratio_add(double D, long long e, long long m)
 {
-    const float p = __fadd_rn(o, __fmul_rn(__fadd_rn((float)i, 0.5f), h));
-    const float g = __fsub_rn(__fdiv_rn(__fsub_rn(p, od), hd), 0.5f);
-    return (g >= -0.5f) && (g < __fsub_rn((float)nd, 0.5f));
+    return m != 0 ? __dadd_rn(D, __dmul_rn(__ddiv_rn((double)e, (double)m), 1.0 / 256.0)) : D;
 }
 
-__global__ void __launch_bounds__(256)
+// Eq. 5 then Eq. 2 per reference voxel.  HBM-bound: (16 n_src + 4) B read + 4 B written per voxel; one thread
+// handles two x-adjacent voxels so the int64 sums move as 128-bit loads (rows are 16-byte aligned when nx is even;
+// odd nx takes the scalar path).
+template <bool kPair>
+__global__ void __launch_bounds__(128)
 emtm_finalize_kernel(const __grid_constant__ FinalizeParams P)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
-    if (i >= P.ref.nx || j >= P.ref.ny) return;
-    const size_t v = ((size_t)k * P.ref.ny + j) * P.ref.nx + i;
-    bool covered = true;
-    for (int s = 0; s < P.n_src && covered; ++s)
-        covered = covered_axis(P.ref.ox, P.ref.hx, i, P.dvf[s].ox, P.dvf[s].hx, P.dvf[s].nx) &&
-                  covered_axis(P.ref.oy, P.ref.hy, j, P.dvf[s].oy, P.dvf[s].hy, P.dvf[s].ny) &&
-                  covered_axis(P.ref.oz, P.ref.hz, k, P.dvf[s].oz, P.dvf[s].hz, P.dvf[s].nz);
-    if (!covered) { P.out[v] = 0.0f; return; }
-    double D = (double)P.dose_ref[v];
-    for (int s = 0; s < P.n_src; ++s) {
-        const long long m = P.M[s][v];
-        if (m != 0) D = __dadd_rn(D, __dmul_rn(__ddiv_rn((double)P.E[s][v], (double)m), 1.0 / 256.0));
+    const int row = blockIdx.x;                          // j + ny * k (grid.x: up to 2^31-1 rows)
+    const int nx = P.ref.nx, ny = P.ref.ny;
+    const int j = row % ny, k = row / ny;
+    const bool row_ok = P.flags[nx + j] && P.flags[nx + ny + k];
+    const size_t base = (size_t)row * nx;
+    if (kPair) {
+        const int i = 2 * (blockIdx.y * blockDim.x + threadIdx.x);
+        if (i >= nx) return;
+        const size_t v = base + i;
+        const bool c0 = row_ok && P.flags[i], c1 = row_ok && P.flags[i + 1];
+        const float2 dr = *reinterpret_cast<const float2*>(P.dose_ref + v);
+        double D0 = (double)dr.x, D1 = (double)dr.y;
+        for (int s = 0; s < P.n_src; ++s) {
+            const longlong2 e = *reinterpret_cast<const longlong2*>(P.E[s] + v);
+            const longlong2 m = *reinterpret_cast<const longlong2*>(P.M[s] + v);
+            D0 = ratio_add(D0, e.x, m.x);
+            D1 = ratio_add(D1, e.y, m.y);
+        }
+        *reinterpret_cast<float2*>(P.out + v) = make_float2(c0 ? (float)D0 : 0.0f, c1 ? (float)D1 : 0.0f);
+    } else {
+        const int i = blockIdx.y * blockDim.x + threadIdx.x;
+        if (i >= nx) return;
+        const size_t v = base + i;
+        double D = (double)P.dose_ref[v];
+        for (int s = 0; s < P.n_src; ++s) D = ratio_add(D, P.E[s][v], P.M[s][v]);
+        P.out[v] = (row_ok && P.flags[i]) ? (float)D : 0.0f;
     }
-    P.out[v] = (float)D;
 }
 
 }  // namespace
 
+void launch_dvf_interleave(const pbs4d_grid& g, const float* disp_planar, float* out4, cudaStream_t st)
+{
+    const size_t n = (size_t)g.nx * g.ny * g.nz;
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 16);
+    dvf_interleave_kernel<<<blocks, 256, 0, st>>>(n, disp_planar, disp_planar + n, disp_planar + 2 * n,
+                                                  reinterpret_cast<float4*>(out4));
+}
+
 void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho, const pbs4d_grid& dvf_grid,
-                      const float* disp, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
+                      const float* disp4, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
                       long long* E, long long* M, AccCounters* counters, cudaStream_t st)
 {
     PushParams P;
     P.src = src; P.dvf = dvf_grid; P.ref = ref; P.dose = dose; P.rho = rho;
-    const size_t plane = (size_t)dvf_grid.nx * dvf_grid.ny * dvf_grid.nz;
-    P.ux = disp; P.uy = disp + plane; P.uz = disp + 2 * plane;
+    P.U = reinterpret_cast<const float4*>(disp4);
     P.nsx = nsx; P.nsy = nsy; P.nsz = nsz;
     P.E = (unsigned long long*)E; P.M = (unsigned long long*)M; P.counters = counters;
-    dim3 b(32, 8, 1), g((src.nx + 31) / 32, (src.ny + 7) / 8, src.nz);
-    emtm_push_kernel<<<g, b, 0, st>>>(P);
+    dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY, src.nz);
+    const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + nsz) * sizeof(AxisEntry);
+    emtm_push_kernel<<<g, b, smem, st>>>(P);
 }
 
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_host,
-                          const long long* const* M_host, const pbs4d_grid* dvf_grids_host, float* out,
-                          cudaStream_t st)
+                          const long long* const* M_host, const pbs4d_grid* dvf_grids_host, unsigned char* flags_dev,
+                          float* out, cudaStream_t st)
 {
+    CoverParams C;
+    C.ref = ref; C.n_src = n_src; C.flags = flags_dev;
+    for (int s = 0; s < n_src && s < kMaxSrc; ++s) C.dvf[s] = dvf_grids_host[s];
+    const int n_axis = ref.nx + ref.ny + ref.nz;
+    emtm_cover_kernel<<<(n_axis + 127) / 128, 128, 0, st>>>(C);
+
     FinalizeParams P;
-    P.ref = ref; P.dose_ref = dose_ref; P.n_src = n_src; P.out = out;
-    for (int s = 0; s < n_src && s < kMaxSrc; ++s) { P.E[s] = E_host[s]; P.M[s] = M_host[s]; P.dvf[s] = dvf_grids_host[s]; }
-    dim3 b(32, 8, 1), g((ref.nx + 31) / 32, (ref.ny + 7) / 8, ref.nz);
-    emtm_finalize_kernel<<<g, b, 0, st>>>(P);
+    P.ref = ref; P.dose_ref = dose_ref; P.n_src = n_src; P.out = out; P.flags = flags_dev;
+    for (int s = 0; s < n_src && s < kMaxSrc; ++s) { P.E[s] = E_host[s]; P.M[s] = M_host[s]; }
+    const bool pair = (ref.nx % 2 == 0) && (reinterpret_cast<uintptr_t>(out) % 8 == 0) &&
+                      (reinterpret_cast<uintptr_t>(dose_ref) % 8 == 0);
+    const int per_row = pair ? ref.nx / 2 : ref.nx;
+    dim3 g(ref.ny * ref.nz, (per_row + 127) / 128);
+    if (pair) emtm_finalize_kernel<true><<<g, 128, 0, st>>>(P);
+    else      emtm_finalize_kernel<false><<<g, 128, 0, st>>>(P);
 }
 
 }  // namespace pbs4d

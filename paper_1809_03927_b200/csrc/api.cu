@@ -79,7 +79,7 @@ struct pbs4d_ctx {
     // accumulation state (a8-a9)
     std::vector<std::unique_ptr<DevBuf>> accE, accM;     // [phase]
     std::vector<bool> have_acc;
-    DevBuf acc_counters;
+    DevBuf acc_counters, cover_flags;
 
     size_t nvox() const { return (size_t)dose_grid.nx * dose_grid.ny * dose_grid.nz; }
 };
@@ -215,9 +215,10 @@ int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pb
     CU(cudaSetDevice(ctx->device));
     auto& d = ctx->dvf[src_phase];
     if (!d.disp) d.disp.reset(new DevBuf);
-    const size_t bytes = (size_t)3 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
+    const size_t bytes = (size_t)4 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
     CU(d.disp->ensure(bytes));
-    CU(cudaMemcpyAsync(d.disp->p, disp_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    launch_dvf_interleave(*dvf_grid, disp_dev, d.disp->as<float>(), ctx->stream);
+    CU(cudaGetLastError());
     CU(cudaStreamSynchronize(ctx->stream));
     d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
     return PBS4D_OK;
@@ -423,8 +424,9 @@ extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int3
         ctx->have_acc[p] = true;
     }
     CU(cudaEventRecord(e1, ctx->stream));
+    CU(ctx->cover_flags.ensure((size_t)ctx->dose_grid.nx + ctx->dose_grid.ny + ctx->dose_grid.nz));
     launch_emtm_finalize(ctx->dose_grid, dose_of(ref_phase), (int)src.size(), Ep.data(), Mp.data(), dg.data(),
-                         dose4d_dev, ctx->stream);
+                         ctx->cover_flags.as<unsigned char>(), dose4d_dev, ctx->stream);
     CU(cudaEventRecord(e2, ctx->stream));
     CU(cudaGetLastError());
     AccCounters ac{};

@@ -50,12 +50,14 @@ void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long
                           double per_protons, float* dose, cudaStream_t st);
 
 struct AccCounters { unsigned long long subvoxels, dropped_ref, dropped_dvf; };
+// planar [3][z][y][x] displacements -> interleaved float4 {ux,uy,uz,0} per node (the layout the push kernel reads)
+void launch_dvf_interleave(const pbs4d_grid& dvf_grid, const float* disp_planar, float* out4, cudaStream_t st);
 void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho, const pbs4d_grid& dvf_grid,
-                      const float* disp, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
+                      const float* disp4, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
                       long long* E, long long* M, AccCounters* counters, cudaStream_t st);
 // out = (first ? dose_ref : out_acc) ... see accumulate.cu: ratio-and-add over all pushed phases, then mask.
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_dev,
-                          const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev, float* out,
-                          cudaStream_t st);
+                          const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev,
+                          unsigned char* flags_dev /*[nx+ny+nz] scratch*/, float* out, cudaStream_t st);
 
 }  // namespace pbs4d
