@@ -48,12 +48,18 @@ __device__ __forceinline__ float lerp_rn(float A, float B, float w)
     return __fadd_rn(A, __fmul_rn(w, __fsub_rn(B, A)));
 }
 
-__device__ __forceinline__ bool dest_index(float q, float o, float h, int n, int& ix)
+// A4: ix = floorf((q - o) / h) with the IEEE quotient, inside iff 0 <= ix < n.  The division is replaced by a
+// multiplication with inv_h = RN(1/h): y = RN(d inv_h) differs from the IEEE quotient RN(d / h) by at most
+// (2^-23 + 2^-24) |y|, so both have the same floor unless y lies within that distance of an integer; in that (rare)
+// case the quotient itself is evaluated.  The result is bit-identical to the plain definition.
+__device__ __forceinline__ float floor_quotient(float d, float h, float inv_h)
 {
-    const float fl = floorf(__fdiv_rn(__fsub_rn(q, o), h));
-    if (!(fl >= 0.0f) || !(fl < (float)n)) return false;
-    ix = (int)fl;
-    return true;
+    const float y  = __fmul_rn(d, inv_h);
+    float fl = floorf(y);
+    const float fr  = __fsub_rn(y, fl);
+    const float tol = __fmul_rn(fabsf(y), 4.0e-7f);
+    if (!(fr >= tol && fr <= __fsub_rn(1.0f, tol))) fl = floorf(__fdiv_rn(d, h));      // also catches NaN/Inf
+    return fl;
 }
 
 // planar [3][N] displacement field -> one float4 {ux, uy, uz, 0} per DVF node, so that a trilinear corner is one
@@ -73,6 +79,7 @@ struct PushParams {
     const float* __restrict__ dose;
     const float* __restrict__ rho;
     const float4* __restrict__ U;            // interleaved DVF
+    float inv_hrx, inv_hry, inv_hrz;         // RN(1 / h) of the reference grid
     int nsx, nsy, nsz;
     unsigned long long* E;
     unsigned long long* M;
@@ -110,26 +117,34 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         const long long m_q = __double2ll_rn(__dmul_rn((double)rho, 16777216.0));
         const long long e_q = __double2ll_rn(__dmul_rn(__dmul_rn((double)rho, (double)dose), 4294967296.0));
         int run_dst = -1, run_cnt = 0;
+        const int nsx = P.nsx, nsy = P.nsy, nsz = P.nsz;
         const int dnx = P.dvf.nx, dny = P.dvf.ny;
+        const int dx1 = dnx > 1 ? 1 : 0;                 // upper x node = lower + 1 unless the DVF grid is 1 node wide
         const float orx = P.ref.ox, ory = P.ref.oy, orz = P.ref.oz, hrx = P.ref.hx, hry = P.ref.hy, hrz = P.ref.hz;
-        const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
-        for (int c = 0; c < P.nsz; ++c) {
+        const float ihx = P.inv_hrx, ihy = P.inv_hry, ihz = P.inv_hrz;
+        const float fnx = (float)P.ref.nx, fny = (float)P.ref.ny, fnz = (float)P.ref.nz;
+        const int rnx = P.ref.nx, rny = P.ref.ny;
+        const AxisEntry* sxl = sx + threadIdx.x;
+        const AxisEntry* syl = sy + threadIdx.y * nsy;
+        for (int c = 0; c < nsz; ++c) {
             const AxisEntry mz = sz[c];
-            for (int b = 0; b < P.nsy; ++b) {
-                const AxisEntry my = sy[threadIdx.y * P.nsy + b];
+            for (int b = 0; b < nsy; ++b) {
+                const AxisEntry my = syl[b];
                 const int r00 = (mz.i0 * dny + my.i0) * dnx;
-                const int r01 = r00 + (my.flags & 1) * dnx;
-                const int r10 = r00 + (mz.flags & 1) * dny * dnx;
-                const int r11 = r10 + (my.flags & 1) * dnx;
+                const int sy1 = (my.flags & 1) * dnx, sz1 = (mz.flags & 1) * dny * dnx;
+                const float4* __restrict__ p00 = P.U + r00;              // the four x-rows of the cell
+                const float4* __restrict__ p01 = p00 + sy1;
+                const float4* __restrict__ p10 = p00 + sz1;
+                const float4* __restrict__ p11 = p10 + sy1;
                 const bool ok_zy = (mz.flags & my.flags & 2) != 0;
-                for (int a = 0; a < P.nsx; ++a) {
-                    const AxisEntry mx = sx[a * kTileX + threadIdx.x];
-                    if (!(ok_zy && (mx.flags & 2))) { n_dvf += 1; continue; }
-                    const int x0 = mx.i0, x1 = mx.i0 + (mx.flags & 1);
-                    const float4 a000 = __ldg(P.U + r00 + x0), a001 = __ldg(P.U + r00 + x1);
-                    const float4 a010 = __ldg(P.U + r01 + x0), a011 = __ldg(P.U + r01 + x1);
-                    const float4 a100 = __ldg(P.U + r10 + x0), a101 = __ldg(P.U + r10 + x1);
-                    const float4 a110 = __ldg(P.U + r11 + x0), a111 = __ldg(P.U + r11 + x1);
+                for (int a = 0; a < nsx; ++a) {
+                    const AxisEntry mx = sxl[a * kTileX];
+                    const bool ok = ok_zy && (mx.flags & 2);
+                    const int x0 = mx.i0;
+                    const float4 a000 = __ldg(p00 + x0), a001 = __ldg(p00 + x0 + dx1);
+                    const float4 a010 = __ldg(p01 + x0), a011 = __ldg(p01 + x0 + dx1);
+                    const float4 a100 = __ldg(p10 + x0), a101 = __ldg(p10 + x0 + dx1);
+                    const float4 a110 = __ldg(p11 + x0), a111 = __ldg(p11 + x0 + dx1);
                     // per component: 4 lerps in x, 2 in y, 1 in z (A3), then q = p + u (A4)
 #define PBS4D_TRILERP(cmp) lerp_rn(lerp_rn(lerp_rn(a000.cmp, a001.cmp, mx.w), lerp_rn(a010.cmp, a011.cmp, mx.w), my.w), \
                                    lerp_rn(lerp_rn(a100.cmp, a101.cmp, mx.w), lerp_rn(a110.cmp, a111.cmp, mx.w), my.w), mz.w)
@@ -137,20 +152,26 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
                     const float qy = __fadd_rn(my.p, PBS4D_TRILERP(y));
                     const float qz = __fadd_rn(mz.p, PBS4D_TRILERP(z));
 #undef PBS4D_TRILERP
-                    int ix, iy, iz;
-                    if (!dest_index(qx, orx, hrx, rnx, ix) || !dest_index(qy, ory, hry, rny, iy) ||
-                        !dest_index(qz, orz, hrz, rnz, iz)) { n_ref += 1; continue; }
-                    const int dst = (iz * rny + iy) * rnx + ix;
-                    if (dst == run_dst) { run_cnt += 1; continue; }
-                    if (run_cnt) {
-                        atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
-                        atomicAdd(P.M + run_dst, (unsigned long long)(run_cnt * m_q));
+                    const float fx = floor_quotient(__fsub_rn(qx, orx), hrx, ihx);
+                    const float fy = floor_quotient(__fsub_rn(qy, ory), hry, ihy);
+                    const float fz = floor_quotient(__fsub_rn(qz, orz), hrz, ihz);
+                    const bool inside = fx >= 0.0f && fx < fnx && fy >= 0.0f && fy < fny && fz >= 0.0f && fz < fnz;
+                    n_dvf += ok ? 0u : 1u;
+                    n_ref += (ok && !inside) ? 1u : 0u;
+                    const int dst = (ok && inside) ? ((int)fz * rny + (int)fy) * rnx + (int)fx : -1;
+                    // merge consecutive subvoxels that land in the same reference voxel into one pair of atomics
+                    if (dst != run_dst) {
+                        if (run_dst >= 0) {
+                            atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
+                            atomicAdd(P.M + run_dst, (unsigned long long)(run_cnt * m_q));
+                        }
+                        run_dst = dst; run_cnt = 0;
                     }
-                    run_dst = dst; run_cnt = 1;
+                    run_cnt += 1;
                 }
             }
         }
-        if (run_cnt) {
+        if (run_dst >= 0) {
             atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
             atomicAdd(P.M + run_dst, (unsigned long long)(run_cnt * m_q));
         }
@@ -262,6 +283,7 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     PushParams P;
     P.src = src; P.dvf = dvf_grid; P.ref = ref; P.dose = dose; P.rho = rho;
     P.U = reinterpret_cast<const float4*>(disp4);
+    P.inv_hrx = 1.0f / ref.hx; P.inv_hry = 1.0f / ref.hy; P.inv_hrz = 1.0f / ref.hz;
     P.nsx = nsx; P.nsy = nsy; P.nsz = nsz;
     P.E = (unsigned long long*)E; P.M = (unsigned long long*)M; P.counters = counters;
     dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY, src.nz);
