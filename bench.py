@@ -23,6 +23,8 @@ sys.path.insert(0, ROOT)
 
 # algorithmic work of one condensed-history step, in fp32/int32 lane-operations
 OPS_PER_STEP = 262
+# dram__bytes_read.sum + dram__bytes_write.sum of one transport_kernel launch (ncu --set full, profiles/)
+TRANSPORT_DRAM_BYTES_PER_LAUNCH = {"config3": 7.6e6}
 
 
 def parse():
@@ -183,16 +185,18 @@ def main():
         ctx.set_plan_spots(cfg["fields"], cfg["spots"])
         deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
         phases = sorted(set(int(x) for x in deliv["segments"]["phase"]) | {cfg["ref_phase"]})
-        n_hist = n_steps = 0
+        n_hist = n_steps = n_red = 0
         t_ms = 0.0
         for p in phases:
             _, _, st = ctx.mc_dose_phase(p, cfg["seed"], want_dose=False)
-            n_hist += st["histories"]; n_steps += st["steps"]; t_ms += st["kernel_ms"]
+            n_hist += st["histories"]; n_steps += st["steps"]; t_ms += st["kernel_ms"]; n_red += st["scoring_atomics"]
         out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
         n_src = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])
-        stats.update(histories=n_hist, mc_steps=n_steps, transport_ms=t_ms, push_ms=ast["push_ms"],
-                     finalize_ms=ast["finalize_ms"], phases=len(phases), n_src=n_src,
-                     launches=P + 2 * len(phases) + n_src + 1, checksum=float(out.sum()))
+        # kernels launched: HU->density per phase, DVF interleave per source phase, transport + dose finalize per
+        # phase run, push per source phase, coverage flags + accumulation finalize
+        stats.update(histories=n_hist, mc_steps=n_steps, reds=n_red, transport_ms=t_ms, push_ms=ast["push_ms"],
+                     finalize_ms=ast["finalize_ms"], phases=len(phases), n_src=n_src, subvoxels=ast["subvoxels"],
+                     launches=P + n_src + 2 * len(phases) + n_src + 2, checksum=float(out.sum()))
         return n_hist
 
     out_host = np.zeros(ctx_shape(cfg), np.float32)
@@ -206,6 +210,9 @@ def main():
         stats["e2e_seconds"] = secs
         return run
 
+    # ---- in-run roofline probes (small kernels of the library itself, before the timed region) ----
+    probes = {k: ctx.roofline_probe(k) for k in ("fp32_issue", "red_random", "red_hot", "hbm_copy")}
+
     # ---- device-resident timing ----
     for _ in range(max(args.warmup, 3)):
         step_device()
@@ -213,9 +220,9 @@ def main():
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    hist = 0; tr_ms = 0.0; mc_steps = 0
+    hist = 0; tr_ms = 0.0; mc_steps = 0; reds = 0
     for _ in range(args.steps):
-        hist += step_device(); tr_ms += stats["transport_ms"]; mc_steps += stats["mc_steps"]
+        hist += step_device(); tr_ms += stats["transport_ms"]; mc_steps += stats["mc_steps"]; reds += stats["reds"]
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
@@ -244,6 +251,9 @@ def main():
     steps_per_s = mc_steps / (tr_ms * 1e-3)
     achieved = steps_per_s * OPS_PER_STEP / 1e12
     props = torch.cuda.get_device_properties(local_rank)
+    nvox = int(np.prod(ctx_shape(cfg)))
+    acc_bytes = stats["n_src"] * nvox * (20 + 16)
+    fin_bytes = nvox * (16 * stats["n_src"] + 8)
     peak = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
     line = {
         "metric": "proton histories/s", "value": hist / (ms * 1e-3), "unit": "histories/s", "n_gpus": world,
@@ -263,9 +273,24 @@ def main():
         "transport_histories_per_s": hist / world / (tr_ms * 1e-3) if world == 1 else None,
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "transport_kernel",
+                     "traffic": TRANSPORT_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "transport_kernel",
                      "how": f"{OPS_PER_STEP} algorithmic lane-ops/step x {steps_per_s:.3e} steps/s over the kernel's CUDA-event "
-                            f"time; peak = SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz, {peak_kind} peaks file)"},
+                            f"time; peak = SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz, {peak_kind} peaks file); "
+                            "traffic = dram bytes read+written per launch from the ncu --set full capture under profiles/",
+                     "measured_fp32_issue": probes["fp32_issue"] / 1e12,
+                     "frac_of_measured_fp32_issue": achieved / (probes["fp32_issue"] / 1e12),
+                     "scoring_atomics_per_s": reds / (tr_ms * 1e-3), "measured_red_random_per_s": probes["red_random"],
+                     "measured_red_hot_per_s": probes["red_hot"],
+                     "atomic_frac": reds / (tr_ms * 1e-3) / probes["red_random"]},
+        "roofline_accumulate": {"bound": "hbm" if max(cfg["subvox"]) <= 2 else "alu", "kernel": "emtm_push_kernel",
+                                "achieved": acc_bytes / (stats["push_ms"] * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                "unit": "GB/s", "frac": acc_bytes / (stats["push_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                "measured_hbm_copy": probes["hbm_copy"] / 1e9,
+                                "subvoxels_per_s": stats["subvoxels"] / (stats["push_ms"] * 1e-3),
+                                "finalize_GBps": fin_bytes / (stats["finalize_ms"] * 1e-3) / 1e9,
+                                "how": "algorithmic bytes = 20 B per source voxel (dose, density, 3 DVF components) + 16 B "
+                                       "read-modify-write per reference voxel, per source phase, over the push kernels' "
+                                       "CUDA-event time; finalize = (16 n_src + 8) B per voxel"},
     }
     if not args.no_cpu_baseline and world == 1:
         r, cores, text = oracle_sample(cfg, 400_000 if args.workload != "config2" else 200_000)

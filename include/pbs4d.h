@@ -80,6 +80,8 @@ typedef struct {
     int64_t  q_incident, q_deposited, q_escaped;        /* fixed point, quantum 2^-fixed_shift MeV */
     int32_t  fixed_shift; int32_t pad;
     float    kernel_ms;                                 /* device time of the transport kernel (CUDA events) */
+    int32_t  pad2;
+    uint64_t scoring_atomics;                           /* red.global.add.u64 issued by the scoring (one per voxel visit) */
 } pbs4d_mc_stats;
 
 typedef struct {
@@ -158,6 +160,20 @@ int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, 
                         const pbs4d_delivery_params* prm, uint64_t total_histories, uint64_t seed,
                         int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
                         double* seconds);
+
+/* In-run roofline probes (BASELINE.json north_star: throughput is reported "as achieved fraction of the FP32-issue,
+ * L2-atomic and HBM roofline measured by in-run microbenchmarks").  Each probe launches a small kernel of its own on
+ * the context's stream, times it with CUDA events (best of 3-5 after a warm-up) and writes one number to *value:
+ *   PBS4D_PROBE_FP32_ISSUE   fp32 FFMA lane-instructions per second (8 independent chains per thread)
+ *   PBS4D_PROBE_RED_RANDOM   red.global.add.u64 lane-atomics per second, random addresses in a 32 MB (L2) window
+ *   PBS4D_PROBE_RED_HOT      the same with one address per warp (the pencil-beam-core case)
+ *   PBS4D_PROBE_HBM_COPY     bytes per second (read + written) of a 1 GiB float4 copy
+ * Temporary device memory (up to 2 GiB for the copy) is allocated and freed inside the call. */
+#define PBS4D_PROBE_FP32_ISSUE  0
+#define PBS4D_PROBE_RED_RANDOM  1
+#define PBS4D_PROBE_RED_HOT     2
+#define PBS4D_PROBE_HBM_COPY    3
+int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value);
 
 #ifdef __cplusplus
 }

@@ -28,7 +28,7 @@ NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
 EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
            "pbs4d_mc_dose_phase", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
-           "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host"]
+           "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe"]
 
 
 class PhaseLists(C.Structure):
@@ -39,10 +39,10 @@ class PhaseLists(C.Structure):
 class McStats(C.Structure):
     _fields_ = [("histories", C.c_uint64), ("steps", C.c_uint64), ("q_incident", C.c_int64),
                 ("q_deposited", C.c_int64), ("q_escaped", C.c_int64), ("fixed_shift", C.c_int32), ("pad", C.c_int32),
-                ("kernel_ms", C.c_float)]
+                ("kernel_ms", C.c_float), ("pad2", C.c_int32), ("scoring_atomics", C.c_uint64)]
 
     def as_dict(self):
-        return {n: getattr(self, n) for n, _ in self._fields_ if n != "pad"}
+        return {n: getattr(self, n) for n, _ in self._fields_ if not n.startswith("pad")}
 
 
 class AccStats(C.Structure):
@@ -225,6 +225,15 @@ class Context:
         self._check(self.lib.pbs4d_get_accumulators(self.h, C.c_int32(src_phase), C.c_void_p(E.data_ptr()),
                                                     C.c_void_p(M.data_ptr())))
         return E, M
+
+    # ---- in-run roofline probes ----
+    PROBES = {"fp32_issue": 0, "red_random": 1, "red_hot": 2, "hbm_copy": 3}
+
+    def roofline_probe(self, kind):
+        """kind: 'fp32_issue' (lane-instr/s), 'red_random' / 'red_hot' (lane-atomics/s), 'hbm_copy' (B/s)"""
+        v = C.c_double(0.0)
+        self._check(self.lib.pbs4d_roofline_probe(self.h, C.c_int32(self.PROBES[kind]), C.byref(v)))
+        return float(v.value)
 
     # ---- whole path, host buffers ----
     def run_plan_host(self, ct_grid, hu_host, dose_grid, dvf_grid, disp_host, ref_phase, fields, spots, prm,

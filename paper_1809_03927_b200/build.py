@@ -13,7 +13,7 @@ INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpbs4d.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
-UNITS = [("api.cu", []), ("transport.cu", []), ("grids.cu", ["-fmad=false"]), ("accumulate.cu", ["-fmad=false"]),
+UNITS = [("api.cu", []), ("transport.cu", []), ("grids.cu", ["-fmad=false"]), ("accumulate.cu", ["-fmad=false"]), ("roofline.cu", []),
          ("delivery.cpp", []), ("tables.cpp", [])]
 
 

@@ -363,6 +363,7 @@ extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed,
         stats->histories = tc.histories; stats->steps = tc.steps;
         stats->q_incident = tc.q_incident; stats->q_deposited = tc.q_deposited; stats->q_escaped = tc.q_escaped;
         stats->fixed_shift = ctx->fixed_shift; stats->pad = 0; stats->kernel_ms = ms;
+        stats->pad2 = 0; stats->scoring_atomics = tc.reds;
     }
     return PBS4D_OK;
 }
@@ -526,5 +527,24 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     const auto t4 = clk::now();
     if (histories_run) *histories_run = run;
     if (seconds) { seconds[0] = sec(t0, t1); seconds[1] = sec(t1, t2); seconds[2] = sec(t2, t3); seconds[3] = sec(t3, t4); }
+    return PBS4D_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// in-run roofline probes
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!value || kind < PBS4D_PROBE_FP32_ISSUE || kind > PBS4D_PROBE_HBM_COPY)
+        return fail(ctx, PBS4D_ERR_ARG, "roofline_probe: bad argument");
+    CU(cudaSetDevice(ctx->device));
+    *value = 0.0;
+    switch (kind) {
+        case PBS4D_PROBE_FP32_ISSUE: CU(probe_fp32_issue(ctx->sm_count, ctx->stream, value)); break;
+        case PBS4D_PROBE_RED_RANDOM: CU(probe_l2_atomic(ctx->sm_count, 0, ctx->stream, value)); break;
+        case PBS4D_PROBE_RED_HOT:    CU(probe_l2_atomic(ctx->sm_count, 1, ctx->stream, value)); break;
+        default:                     CU(probe_hbm_copy(ctx->sm_count, ctx->stream, value)); break;
+    }
     return PBS4D_OK;
 }

@@ -36,6 +36,7 @@ struct TransportCounters {       // device tallies of one launch (zeroed before 
     unsigned long long histories, steps;
     long long q_incident, q_deposited, q_escaped;
     unsigned long long next_history;      // work counter: next local history index to hand out
+    unsigned long long reds;              // scoring atomics issued
 };
 
 // Launchers (all asynchronous on `st`).
@@ -59,5 +60,12 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_dev,
                           const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev,
                           unsigned char* flags_dev /*[nx+ny+nz] scratch*/, float* out, cudaStream_t st);
+
+// ---- in-run roofline probes (roofline.cu) ----
+#ifdef __CUDACC__
+cudaError_t probe_fp32_issue(int sm_count, cudaStream_t st, double* lane_inst_per_s);
+cudaError_t probe_l2_atomic(int sm_count, int hot, cudaStream_t st, double* lane_atomics_per_s);
+cudaError_t probe_hbm_copy(int sm_count, cudaStream_t st, double* bytes_per_s);
+#endif
 
 }  // namespace pbs4d

@@ -195,8 +195,9 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
     return true;
 }
 
-__device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep)
+__device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep, uint32_t& n_red)
 {
+    n_red += 1u;
     atomicAdd(P.Q + L.vox, (unsigned long long)L.pend);
     q_dep += L.pend;
     L.pend = 0;
@@ -206,14 +207,14 @@ __global__ void __launch_bounds__(kThreads)
 transport_kernel(const __grid_constant__ Params P)
 {
     __shared__ float4 s_tab[kTabNodes];
-    __shared__ long long s_tally[5];
+    __shared__ long long s_tally[6];
     for (int i = threadIdx.x; i < kTabNodes; i += kThreads) s_tab[i] = P.tab[i];
-    if (threadIdx.x < 5) s_tally[threadIdx.x] = 0;
+    if (threadIdx.x < 6) s_tally[threadIdx.x] = 0;
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u;
     long long q_inc = 0, q_dep = 0, q_esc = 0;
-    uint32_t n_steps = 0, n_hist = 0;
+    uint32_t n_steps = 0, n_hist = 0, n_red = 0;
     const float hx = P.g.hx, hy = P.g.hy, hz = P.g.hz;
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
     const bool do_mcs = !(P.flags & PBS4D_NO_MCS), do_strag = !(P.flags & PBS4D_NO_STRAGGLE);
@@ -335,7 +336,7 @@ transport_kernel(const __grid_constant__ Params P)
             L.E -= dE;
 
             if (crossing || !alive) {
-                flush(P, L, q_dep);
+                flush(P, L, q_dep, n_red);
                 if (alive) {
                     if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
                         q_esc += __double2ll_rn((double)L.E * L.wq_d);                       // left the grid
@@ -351,17 +352,18 @@ transport_kernel(const __grid_constant__ Params P)
     }
 
     // block-level tally reduction: warp shuffle, shared atomics, one global atomic per block and counter
-    long long v[5] = { (long long)n_hist, (long long)n_steps, q_inc, q_dep, q_esc };
+    long long v[6] = { (long long)n_hist, (long long)n_steps, q_inc, q_dep, q_esc, (long long)n_red };
 #pragma unroll
-    for (int c = 0; c < 5; ++c) {
+    for (int c = 0; c < 6; ++c) {
         long long x = v[c];
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
         if (lane == 0) atomicAdd((unsigned long long*)&s_tally[c], (unsigned long long)x);
     }
     __syncthreads();
-    if (threadIdx.x < 5) {
-        unsigned long long* dst = threadIdx.x == 0 ? &P.counters->histories
+    if (threadIdx.x < 6) {
+        unsigned long long* dst = threadIdx.x == 5 ? &P.counters->reds
+                                : threadIdx.x == 0 ? &P.counters->histories
                                 : threadIdx.x == 1 ? &P.counters->steps
                                 : threadIdx.x == 2 ? (unsigned long long*)&P.counters->q_incident
                                 : threadIdx.x == 3 ? (unsigned long long*)&P.counters->q_deposited

@@ -31,7 +31,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_the_header():
     assert binding.GRID_DT.itemsize == 36 and binding.FIELD_DT.itemsize == 52 and binding.SPOT_DT.itemsize == 28
     assert binding.DELIV_DT.itemsize == 56 and binding.SEG_DT.itemsize == 48
-    assert C.sizeof(binding.McStats) == 56 and C.sizeof(binding.AccStats) == 32
+    assert C.sizeof(binding.McStats) == 64 and C.sizeof(binding.AccStats) == 32
     for a, b in [(binding.GRID_DT, synth.GRID_DT), (binding.FIELD_DT, synth.FIELD_DT), (binding.SPOT_DT, synth.SPOT_DT),
                  (binding.DELIV_DT, synth.DELIV_DT)]:
         assert a == b
