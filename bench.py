@@ -24,7 +24,7 @@ sys.path.insert(0, ROOT)
 # algorithmic work of one condensed-history step, in fp32/int32 lane-operations
 OPS_PER_STEP = 262
 # dram__bytes_read.sum + dram__bytes_write.sum of one transport_kernel launch (ncu --set full, profiles/)
-TRANSPORT_DRAM_BYTES_PER_LAUNCH = {"config3": 7.6e6}
+TRANSPORT_DRAM_BYTES_PER_LAUNCH = {"config3": 7.6e6, "config5": 74.8e6}
 
 
 def parse():
