@@ -24,6 +24,8 @@ sys.path.insert(0, ROOT)
 # algorithmic work of one condensed-history step, in fp32/int32 lane-operations
 OPS_PER_STEP = 262
 # dram__bytes_read.sum + dram__bytes_write.sum of one transport_kernel launch (ncu --set full, profiles/)
+# histories of the bounded oracle sample (10-30 s of host work on 16 cores); the reference arm uses half per step
+ORACLE_SAMPLE = {"config5": 200_000, "config3": 400_000, "config2": 200_000}
 TRANSPORT_DRAM_BYTES_PER_LAUNCH = {"config3": 7.6e6, "config5": 74.8e6}
 
 
@@ -118,12 +120,26 @@ def oracle_sample(cfg, budget_hist):
                              f"(delivery + HU->density + transport; {wall:.1f} s wall, transport {t_tr:.1f} s)")
 
 
+def reduce_over_ranks(ms, e2e_s, hist, hist_e2e, world, device):
+    """Replicas: every rank ran an independent plan.  Times -> MAX over ranks, histories -> SUM over ranks
+    (whole-job throughput = all histories / slowest rank's time).  The only collectives of the whole program."""
+    if world <= 1:
+        return ms, e2e_s, hist, hist_e2e
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=device)
+    n = torch.tensor([float(hist), float(hist_e2e)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(n[0]), float(n[1])
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
     if rank != 0:
         return
     cfg = make_workload(args.workload, 0, args.histories)
-    budget = 400_000 if args.workload != "config2" else 200_000
+    budget = ORACLE_SAMPLE[args.workload] // 2
     rates, text, cores = [], "", 0
     for i in range(args.warmup + args.steps):
         r, cores, text = oracle_sample(cfg, budget)
@@ -238,11 +254,7 @@ def main():
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    tvals = torch.tensor([ms, e2e_s, float(hist), float(hist_e2e)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = tvals.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = tvals.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms, e2e_s, hist, hist_e2e = float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
+    ms, e2e_s, hist, hist_e2e = reduce_over_ranks(ms, e2e_s, hist, hist_e2e, world, torch.device("cuda", local_rank))
     if rank != 0:
         return
 
@@ -293,7 +305,7 @@ def main():
                                        "CUDA-event time; finalize = (16 n_src + 8) B per voxel"},
     }
     if not args.no_cpu_baseline and world == 1:
-        r, cores, text = oracle_sample(cfg, 400_000 if args.workload != "config2" else 200_000)
+        r, cores, text = oracle_sample(cfg, ORACLE_SAMPLE[args.workload])
         line["cpu_baseline"] = {"value": r, "unit": "histories/s", "cores": cores, "kind": "oracle", "sample": text}
     print(json.dumps(line), flush=True)
     ctx.close()
