@@ -29,7 +29,9 @@ namespace pbs4d {
 
 namespace {
 
-constexpr int   kThreads   = 128;
+constexpr int   kThreads   = 256;
+constexpr int   kWarps     = kThreads / 32;
+constexpr int   kPoolWords = 10;                                     // words per pre-sampled history in the warp's pool
 constexpr float kEcut      = 0.5f;
 constexpr float kSmax      = 1.0f;
 constexpr float kTie       = 1.0f + 1.0f / 1024.0f;                  // boundary/step-limit tie tolerance (DESIGN A22)
@@ -123,6 +125,7 @@ struct Lane {
     int vox;                                   // linear voxel index of the pending deposit (< 2^31 voxels)
     long long pend;                            // quanta deposited in vox and not yet flushed
     float dens, inv_dens;
+    int seg;                                   // index of the history's segment in the launch table
 };
 
 // T3: sample history j of the launch.  Returns false if the ray misses the grid (all energy escapes).
@@ -135,6 +138,7 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
         if (__ldg(P.seg_begin + mid) <= j) lo = mid; else hi = mid - 1;
     }
     const DevSegment& S = P.segs[lo];
+    L.seg = lo;
     const unsigned long long g = (unsigned long long)(S.first_history + (j - S.local_begin));
     L.g_lo = (uint32_t)g; L.g_hi = (uint32_t)(g >> 32); L.m = 0u;
     L.wq = S.weight_scaled; L.wq_d = S.weight_scaled_d;
@@ -190,8 +194,6 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
     L.ix = idx[0]; L.iy = idx[1]; L.iz = idx[2];
     L.vox = (L.iz * P.g.ny + L.iy) * P.g.nx + L.ix;
     L.pend = 0;
-    L.dens = __ldg(P.rho + L.vox);
-    L.inv_dens = fast_rcp(L.dens);
     return true;
 }
 
@@ -203,11 +205,12 @@ __device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep
     L.pend = 0;
 }
 
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 4)
 transport_kernel(const __grid_constant__ Params P)
 {
     __shared__ float4 s_tab[kTabNodes];
     __shared__ long long s_tally[6];
+    __shared__ uint32_t s_pool[kWarps][kPoolWords][32];
     for (int i = threadIdx.x; i < kTabNodes; i += kThreads) s_tab[i] = P.tab[i];
     if (threadIdx.x < 6) s_tally[threadIdx.x] = 0;
     __syncthreads();
@@ -219,25 +222,66 @@ transport_kernel(const __grid_constant__ Params P)
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
     const bool do_mcs = !(P.flags & PBS4D_NO_MCS), do_strag = !(P.flags & PBS4D_NO_STRAGGLE);
 
+    // Per-warp pool of 32 pre-sampled histories (T3 done by the whole warp at once, at full lane efficiency); a lane
+    // whose history ends pops the next one instead of sampling it alone while 31 lanes wait.
+    uint32_t (*pool)[32] = s_pool[threadIdx.x >> 5];
+    int  avail = 0;                                     // warp-uniform: unconsumed pool entries (32-avail .. 31)
+    bool drained = false;                               // warp-uniform: the launch has no histories left to fetch
+
     Lane L;
     bool alive = false, exhausted = false;
     for (;;) {
-        // ---------------- refill phase: dead lanes take the next history indices of the launch ----------------
-        const unsigned want = __ballot_sync(0xffffffffu, !alive && !exhausted);
-        if (want) {
-            const int leader = __ffs(want) - 1;
-            unsigned long long base = 0;
-            if (lane == (unsigned)leader) base = atomicAdd(&P.counters->next_history, (unsigned long long)__popc(want));
-            base = __shfl_sync(0xffffffffu, base, leader);
-            if (!alive && !exhausted) {
-                const long long j = (long long)base + __popc(want & ((1u << lane) - 1u));
+        // ---------------- refill phase: dead lanes pop pre-sampled histories ----------------
+        const bool dead = !alive && !exhausted;
+        const unsigned need = __ballot_sync(0xffffffffu, dead);
+        if (need) {
+            if (avail == 0 && !drained) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(&P.counters->next_history, 32ull);
+                base = __shfl_sync(0xffffffffu, base, 0);
+                const long long j = (long long)base + lane;
+                int tag = -1;                           // -1: no such history, -2: the ray misses the grid
                 if (j < P.n_hist) {
-                    Lane T;                                   // the out-of-line call writes a stack temporary;
-                    long long qi = 0, qe = 0;                 // the loop's own state stays in registers
-                    alive = start_history(P, j, T, qi, qe);
-                    L = T; q_inc += qi; q_esc += qe; n_hist += 1;
+                    Lane T;
+                    long long qi = 0, qe = 0;
+                    const bool ok = start_history(P, j, T, qi, qe);
+                    q_inc += qi; q_esc += qe; n_hist += 1;
+                    tag = ok ? T.seg : -2;
+                    pool[0][lane] = __float_as_uint(T.px); pool[1][lane] = __float_as_uint(T.py);
+                    pool[2][lane] = __float_as_uint(T.pz); pool[3][lane] = __float_as_uint(T.E);
+                    pool[4][lane] = (uint32_t)T.ix; pool[5][lane] = (uint32_t)T.iy; pool[6][lane] = (uint32_t)T.iz;
+                    pool[7][lane] = T.g_lo; pool[8][lane] = T.g_hi;
                 }
-                else exhausted = true;
+                pool[9][lane] = (uint32_t)tag;
+                drained = (long long)base + 32 >= P.n_hist;
+                avail = 32;
+                __syncwarp();
+            }
+            if (avail > 0) {
+                const int rank = __popc(need & ((1u << lane) - 1u));
+                if (dead && rank < avail) {
+                    const int sl = 32 - avail + rank;
+                    const int tag = (int)pool[9][sl];
+                    if (tag == -1) exhausted = true;
+                    else if (tag >= 0) {
+                        const DevSegment& S = P.segs[tag];
+                        L.px = __uint_as_float(pool[0][sl]); L.py = __uint_as_float(pool[1][sl]);
+                        L.pz = __uint_as_float(pool[2][sl]); L.E  = __uint_as_float(pool[3][sl]);
+                        L.ix = (int)pool[4][sl]; L.iy = (int)pool[5][sl]; L.iz = (int)pool[6][sl];
+                        L.g_lo = pool[7][sl]; L.g_hi = pool[8][sl]; L.m = 0u;
+                        L.dx = S.dir[0]; L.dy = S.dir[1]; L.dz = S.dir[2];
+                        L.wq = S.weight_scaled; L.wq_d = S.weight_scaled_d;
+                        L.vox = (L.iz * ny + L.iy) * nx + L.ix;
+                        L.pend = 0;
+                        L.dens = __ldg(P.rho + L.vox);
+                        L.inv_dens = fast_rcp(L.dens);
+                        alive = true;
+                    }
+                }
+                avail = max(avail - __popc(need), 0);
+                __syncwarp();
+            } else if (dead) {
+                exhausted = true;                       // pool empty and nothing left to fetch
             }
         }
         if (!__any_sync(0xffffffffu, alive)) {
