@@ -119,7 +119,6 @@ __device__ __forceinline__ Lookup locate(float E)
 // Per-lane history state.  Position p* is voxel-local: 0 <= p <= h on each axis.
 struct Lane {
     float px, py, pz, dx, dy, dz, E, wq;      // wq = weight * 2^k (deposit -> quanta)
-    double wq_d;
     int ix, iy, iz;
     uint32_t g_lo, g_hi, m;
     int vox;                                   // linear voxel index of the pending deposit (< 2^31 voxels)
@@ -141,7 +140,7 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
     L.seg = lo;
     const unsigned long long g = (unsigned long long)(S.first_history + (j - S.local_begin));
     L.g_lo = (uint32_t)g; L.g_hi = (uint32_t)(g >> 32); L.m = 0u;
-    L.wq = S.weight_scaled; L.wq_d = S.weight_scaled_d;
+    L.wq = S.weight_scaled;
 
     uint32_t r0, r1, r2, r3;
     philox(P, 0u, L.g_lo, L.g_hi, r0, r1, r2, r3);
@@ -158,7 +157,7 @@ __device__ __noinline__ bool start_history(const Params& P, long long j, Lane& L
     float r[3], d[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) { r[k] = S.ref[k] + a * S.eu[k] + b * S.ev[k]; d[k] = S.dir[k]; }
-    const long long qi = __double2ll_rn((double)L.E * L.wq_d);
+    const long long qi = __double2ll_rn((double)L.E * S.weight_scaled_d);
     q_inc += qi;
 
     // slab-method ray/box intersection over t in (-inf, inf)
@@ -216,8 +215,8 @@ transport_kernel(const __grid_constant__ Params P)
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u;
-    long long q_inc = 0, q_dep = 0, q_esc = 0;
-    uint32_t n_steps = 0, n_hist = 0, n_red = 0;
+    long long q_dep = 0;                                // rare tallies (incident, escaped, histories) go straight to
+    uint32_t n_steps = 0, n_red = 0;                    // shared memory; per-step ones stay in registers
     const float hx = P.g.hx, hy = P.g.hy, hz = P.g.hz;
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
     const bool do_mcs = !(P.flags & PBS4D_NO_MCS), do_strag = !(P.flags & PBS4D_NO_STRAGGLE);
@@ -245,7 +244,9 @@ transport_kernel(const __grid_constant__ Params P)
                     Lane T;
                     long long qi = 0, qe = 0;
                     const bool ok = start_history(P, j, T, qi, qe);
-                    q_inc += qi; q_esc += qe; n_hist += 1;
+                    atomicAdd((unsigned long long*)&s_tally[0], 1ull);
+                    atomicAdd((unsigned long long*)&s_tally[2], (unsigned long long)qi);
+                    if (qe) atomicAdd((unsigned long long*)&s_tally[4], (unsigned long long)qe);
                     tag = ok ? T.seg : -2;
                     pool[0][lane] = __float_as_uint(T.px); pool[1][lane] = __float_as_uint(T.py);
                     pool[2][lane] = __float_as_uint(T.pz); pool[3][lane] = __float_as_uint(T.E);
@@ -270,7 +271,7 @@ transport_kernel(const __grid_constant__ Params P)
                         L.ix = (int)pool[4][sl]; L.iy = (int)pool[5][sl]; L.iz = (int)pool[6][sl];
                         L.g_lo = pool[7][sl]; L.g_hi = pool[8][sl]; L.m = 0u;
                         L.dx = S.dir[0]; L.dy = S.dir[1]; L.dz = S.dir[2];
-                        L.wq = S.weight_scaled; L.wq_d = S.weight_scaled_d;
+                        L.wq = S.weight_scaled; L.seg = tag;
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.pend = 0;
                         L.dens = __ldg(P.rho + L.vox);
@@ -383,7 +384,8 @@ transport_kernel(const __grid_constant__ Params P)
                 flush(P, L, q_dep, n_red);
                 if (alive) {
                     if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
-                        q_esc += __double2ll_rn((double)L.E * L.wq_d);                       // left the grid
+                        atomicAdd((unsigned long long*)&s_tally[4],                            // left the grid
+                                  (unsigned long long)__double2ll_rn((double)L.E * P.segs[L.seg].weight_scaled_d));
                         alive = false;
                     } else {
                         L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
@@ -396,7 +398,7 @@ transport_kernel(const __grid_constant__ Params P)
     }
 
     // block-level tally reduction: warp shuffle, shared atomics, one global atomic per block and counter
-    long long v[6] = { (long long)n_hist, (long long)n_steps, q_inc, q_dep, q_esc, (long long)n_red };
+    long long v[6] = { 0, (long long)n_steps, 0, q_dep, 0, (long long)n_red };
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
         long long x = v[c];
