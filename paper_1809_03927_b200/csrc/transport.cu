@@ -38,7 +38,7 @@ constexpr float kTie       = 1.0f + 1.0f / 1024.0f;                  // boundary
 constexpr float kTwoPi     = 6.283185307179586f;
 constexpr float kPi        = 3.14159265358979f;
 constexpr float kNeg2Ln2   = -1.3862943611198906f;                  // -2 ln 2
-constexpr float kHuge      = 1.0e30f;
+constexpr float kTinyDir   = 1.0e-20f;                              // stands in for an exactly-zero direction component
 
 struct Params {
     pbs4d_grid g;
@@ -271,7 +271,9 @@ transport_kernel(const __grid_constant__ Params P)
                         L.pz = __uint_as_float(pool[2][sl]); L.E  = __uint_as_float(pool[3][sl]);
                         L.ix = (int)pool[4][sl]; L.iy = (int)pool[5][sl]; L.iz = (int)pool[6][sl];
                         L.g_lo = pool[7][sl]; L.g_hi = pool[8][sl]; L.m = 0u;
-                        L.dx = S.dir[0]; L.dy = S.dir[1]; L.dz = S.dir[2];
+                        L.dx = S.dir[0] == 0.0f ? kTinyDir : S.dir[0];
+                        L.dy = S.dir[1] == 0.0f ? kTinyDir : S.dir[1];
+                        L.dz = S.dir[2] == 0.0f ? kTinyDir : S.dir[2];
                         L.wq = S.weight_scaled; L.seg = tag;
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.pend = 0;
@@ -302,13 +304,12 @@ transport_kernel(const __grid_constant__ Params P)
 
             // T6: nearest voxel face.  Per axis: numerator = distance to the face ahead, denominator = |d|;
             // the smallest quotient is found by cross-multiplication, then one reciprocal.
-            float numx = L.dx > 0.0f ? hx - L.px : L.px, denx = fabsf(L.dx);
-            float numy = L.dy > 0.0f ? hy - L.py : L.py, deny = fabsf(L.dy);
-            float numz = L.dz > 0.0f ? hz - L.pz : L.pz, denz = fabsf(L.dz);
-            numx = fmaxf(numx, 0.0f); numy = fmaxf(numy, 0.0f); numz = fmaxf(numz, 0.0f);
-            if (denx == 0.0f) { numx = kHuge; denx = 1.0f; }
-            if (deny == 0.0f) { numy = kHuge; deny = 1.0f; }
-            if (denz == 0.0f) { numz = kHuge; denz = 1.0f; }
+            // (direction components are never exactly zero: a zero component of the field direction is replaced by
+            // +1e-20 when the history starts, which keeps that axis' quotient astronomically large, as 1/0 would)
+            const float denx = fabsf(L.dx), deny = fabsf(L.dy), denz = fabsf(L.dz);
+            const float numx = fmaxf(L.dx > 0.0f ? hx - L.px : L.px, 0.0f);
+            const float numy = fmaxf(L.dy > 0.0f ? hy - L.py : L.py, 0.0f);
+            const float numz = fmaxf(L.dz > 0.0f ? hz - L.pz : L.pz, 0.0f);
             // x against z, then y against the winner; equal cross products mark axes that attain the minimum together
             const float cxz = numx * denz, czx = numz * denx;
             const bool  x_lt = cxz < czx;
