@@ -201,11 +201,9 @@ def main():
         ctx.set_plan_spots(cfg["fields"], cfg["spots"])
         deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
         phases = sorted(set(int(x) for x in deliv["segments"]["phase"]) | {cfg["ref_phase"]})
-        n_hist = n_steps = n_red = 0
-        t_ms = 0.0
-        for p in phases:
-            _, _, st = ctx.mc_dose_phase(p, cfg["seed"], want_dose=False)
-            n_hist += st["histories"]; n_steps += st["steps"]; t_ms += st["kernel_ms"]; n_red += st["scoring_atomics"]
+        sts, t_ms = ctx.mc_dose_phases(phases, cfg["seed"])          # all phases, concurrent launches; t_ms = fork..join
+        n_hist = sum(st["histories"] for st in sts); n_steps = sum(st["steps"] for st in sts)
+        n_red = sum(st["scoring_atomics"] for st in sts)
         out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
         n_src = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])
         # kernels launched: HU->density per phase, DVF interleave per source phase, transport + dose finalize per
@@ -286,8 +284,8 @@ def main():
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
                      "traffic": TRANSPORT_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "transport_kernel",
-                     "how": f"{OPS_PER_STEP} algorithmic lane-ops/step x {steps_per_s:.3e} steps/s over the kernel's CUDA-event "
-                            f"time; peak = SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz, {peak_kind} peaks file); "
+                     "how": f"{OPS_PER_STEP} algorithmic lane-ops/step x {steps_per_s:.3e} steps/s over the CUDA-event time of the "
+                            f"transport launches of a pass (fork to join of the per-phase kernels, which overlap at their tails); peak = SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz, {peak_kind} peaks file); "
                             "traffic = dram bytes read+written per launch from the ncu --set full capture under profiles/",
                      "measured_fp32_issue": probes["fp32_issue"] / 1e12,
                      "frac_of_measured_fp32_issue": achieved / (probes["fp32_issue"] / 1e12),

@@ -137,6 +137,14 @@ int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field* fields, in
 int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
                         float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats);
 
+/* The same for n distinct phases at once ("N_g simulations per field", one per breathing phase; the
+ * paper spread them over its 8 cards, here they share one device): the n transport kernels are enqueued on internal
+ * streams between a fork and a join on the context's stream, so the drain of one persistent kernel overlaps the next.
+ * stats (optional) -> [n], in the order of `phases`; kernel_ms of overlapping launches overlap too, so *elapsed_ms
+ * (optional) receives the device time from fork to join.  Results are identical to n mc_dose_phase calls. */
+int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* phases, uint64_t seed, double per_protons,
+                         pbs4d_mc_stats* stats, float* elapsed_ms);
+
 /* Fixed-point energy grid of the last mc_dose_phase call for `phase`, copied to q_dev (int64 [z][y][x]). */
 int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev);
 

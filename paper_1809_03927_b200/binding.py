@@ -27,7 +27,7 @@ NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
 
 EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
-           "pbs4d_mc_dose_phase", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
+           "pbs4d_mc_dose_phase", "pbs4d_mc_dose_phases", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
            "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe"]
 
 
@@ -198,6 +198,17 @@ class Context:
                                                  C.c_void_p(dose.data_ptr() if want_dose else None),
                                                  C.c_void_p(rho.data_ptr() if want_rho else None), C.byref(st)))
         return dose, rho, st.as_dict()
+
+    def mc_dose_phases(self, phases, seed, per_protons=0.0):
+        """all listed phases in one call (concurrent launches); -> (list of stats dicts, device ms fork..join);
+        the doses stay in the context (accumulate_subvoxel / get_phase_energy)"""
+        n = len(phases)
+        arr = (C.c_int32 * n)(*[int(p) for p in phases])
+        st = (McStats * n)()
+        ms = C.c_float(0.0)
+        self._check(self.lib.pbs4d_mc_dose_phases(self.h, C.c_int32(n), arr, C.c_uint64(int(seed)),
+                                                  C.c_double(float(per_protons)), st, C.byref(ms)))
+        return [s.as_dict() for s in st], float(ms.value)
 
     def get_phase_energy(self, phase):
         t = self.torch

@@ -74,12 +74,15 @@ struct pbs4d_ctx {
     std::vector<std::unique_ptr<DevBuf>> q;              // [phase] int64 energy grid
     std::vector<std::unique_ptr<DevBuf>> dose;           // [phase] fp32 Gy
     std::vector<bool> have_dose;
-    DevBuf seg_dev, counters;
+    DevBuf counters;
+    std::vector<std::unique_ptr<DevBuf>> seg_phase;      // [phase] launch table (DevSegment[] | seg_begin[])
+    std::vector<cudaStream_t> aux;                       // auxiliary streams for concurrent phase launches
 
     // accumulation state (a8-a9)
     std::vector<std::unique_ptr<DevBuf>> accE, accM;     // [phase]
     std::vector<bool> have_acc;
     DevBuf acc_counters, cover_flags;
+    DevBuf host_hu, host_dvf, host_out;                  // staging buffers of run_plan_host, kept across calls
 
     size_t nvox() const { return (size_t)dose_grid.nx * dose_grid.ny * dose_grid.nz; }
 };
@@ -150,6 +153,7 @@ void pbs4d_destroy(pbs4d_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    for (auto st : ctx->aux) if (st) cudaStreamDestroy(st);
     delete ctx;
 }
 
@@ -315,56 +319,115 @@ extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_para
 // ------------------------------------------------------------------------------------------------------------------
 // a4-a7: transport + scoring + finalize for one phase
 // ------------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr int kAuxStreams = 4;
+}
+
+extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* phases, uint64_t seed, double per_protons,
+                                    pbs4d_mc_stats* stats, float* elapsed_ms)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: no densities (set_ct_phases)");
+    if (!ctx->have_delivery) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: call simulate_delivery first");
+    if (n < 1 || n > 32 || !phases) return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phases: bad argument");
+    for (int a = 0; a < n; ++a) {
+        if (phases[a] < 0 || phases[a] >= ctx->n_phases || phases[a] >= ctx->deliv_phases)
+            return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phases: phase out of range");
+        for (int b = 0; b < a; ++b)
+            if (phases[b] == phases[a]) return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phases: phase listed twice");
+    }
+    CU(cudaSetDevice(ctx->device));
+    const size_t nvox = ctx->nvox();
+    // streams: one launch alone runs on the context's stream; several run on auxiliary streams between a fork and a
+    // join event so that the tail of one phase's persistent kernel overlaps the start of the next
+    const bool fan_out = n > 1;
+    if (fan_out && ctx->aux.empty()) {
+        ctx->aux.resize(kAuxStreams, nullptr);
+        for (auto& st : ctx->aux) CU(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    }
+    if (ctx->seg_phase.size() < (size_t)ctx->n_phases) {
+        ctx->seg_phase.resize(ctx->n_phases);
+        for (auto& b : ctx->seg_phase) if (!b) b.reset(new DevBuf);
+    }
+    CU(ctx->counters.ensure(sizeof(TransportCounters) * 32));
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(TransportCounters) * n, ctx->stream));
+    std::vector<cudaEvent_t> ev(2 * n + 2 + kAuxStreams, nullptr);
+    auto destroy_events = [&] { for (auto e : ev) if (e) cudaEventDestroy(e); };
+    for (auto& e : ev) {
+        cudaError_t ce = cudaEventCreate(&e);
+        if (ce != cudaSuccess) { destroy_events(); return cuda_fail(ctx, ce, "cudaEventCreate"); }
+    }
+    cudaEvent_t span0 = ev[2 * n], span1 = ev[2 * n + 1];
+    int rc = PBS4D_OK;
+    auto guard = [&](cudaError_t ce, const char* what) { if (ce != cudaSuccess && rc == PBS4D_OK) rc = cuda_fail(ctx, ce, what); };
+    guard(cudaEventRecord(span0, ctx->stream), "record");
+    if (fan_out) for (auto st : ctx->aux) guard(cudaStreamWaitEvent(st, span0, 0), "fork");
+    for (int a = 0; a < n && rc == PBS4D_OK; ++a) {
+        const int phase = phases[a];
+        cudaStream_t st = fan_out ? ctx->aux[a % kAuxStreams] : ctx->stream;
+        PhaseLaunch& L = ctx->launches[phase];
+        guard(ctx->q[phase]->ensure(nvox * sizeof(long long)), "alloc energy grid");
+        guard(ctx->dose[phase]->ensure(nvox * sizeof(float)), "alloc dose grid");
+        if (rc != PBS4D_OK) break;
+        guard(cudaMemsetAsync(ctx->q[phase]->p, 0, nvox * sizeof(long long), st), "memset");
+        guard(cudaEventRecord(ev[2 * a], st), "record");
+        if (L.n_hist > 0) {
+            DevBuf& sb = *ctx->seg_phase[phase];
+            const size_t seg_bytes = L.segs.size() * sizeof(DevSegment);
+            guard(sb.ensure(seg_bytes + L.segs.size() * sizeof(long long)), "alloc segments");
+            if (rc != PBS4D_OK) break;
+            guard(cudaMemcpyAsync(sb.p, L.segs.data(), seg_bytes, cudaMemcpyHostToDevice, st), "segments H2D");
+            guard(cudaMemcpyAsync(sb.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
+                                  cudaMemcpyHostToDevice, st), "segments H2D");
+            guard(cudaEventRecord(ev[2 * a], st), "record");
+            launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), sb.as<DevSegment>(),
+                             reinterpret_cast<const long long*>(sb.as<char>() + seg_bytes), (int32_t)L.segs.size(),
+                             L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
+                             ctx->counters.as<TransportCounters>() + a, ctx->sm_count, st);
+        }
+        guard(cudaEventRecord(ev[2 * a + 1], st), "record");
+        launch_finalize_dose(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->q[phase]->as<long long>(),
+                             ctx->fixed_shift, per_protons, ctx->dose[phase]->as<float>(), st);
+        guard(cudaGetLastError(), "launch");
+    }
+    if (fan_out) {
+        for (int k = 0; k < kAuxStreams; ++k) {
+            guard(cudaEventRecord(ev[2 * n + 2 + k], ctx->aux[k]), "record");
+            guard(cudaStreamWaitEvent(ctx->stream, ev[2 * n + 2 + k], 0), "join");
+        }
+    }
+    guard(cudaEventRecord(span1, ctx->stream), "record");
+    std::vector<TransportCounters> tc(n);
+    guard(cudaMemcpyAsync(tc.data(), ctx->counters.p, sizeof(TransportCounters) * n, cudaMemcpyDeviceToHost, ctx->stream),
+          "counters D2H");
+    guard(cudaStreamSynchronize(ctx->stream), "synchronize");
+    if (rc == PBS4D_OK) {
+        for (int a = 0; a < n; ++a) {
+            ctx->have_dose[phases[a]] = true;
+            if (!stats) continue;
+            pbs4d_mc_stats& s = stats[a];
+            s.histories = tc[a].histories; s.steps = tc[a].steps;
+            s.q_incident = tc[a].q_incident; s.q_deposited = tc[a].q_deposited; s.q_escaped = tc[a].q_escaped;
+            s.fixed_shift = ctx->fixed_shift; s.pad = 0; s.pad2 = 0; s.scoring_atomics = tc[a].reds;
+            s.kernel_ms = 0.0f;
+            cudaEventElapsedTime(&s.kernel_ms, ev[2 * a], ev[2 * a + 1]);
+        }
+        if (elapsed_ms) cudaEventElapsedTime(elapsed_ms, span0, span1);
+    }
+    destroy_events();
+    return rc;
+}
+
 extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
                                    float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats)
 {
     if (!ctx) return PBS4D_ERR_ARG;
-    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phase: no densities (set_ct_phases)");
-    if (!ctx->have_delivery) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phase: call simulate_delivery first");
-    if (phase < 0 || phase >= ctx->n_phases || phase >= ctx->deliv_phases)
-        return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phase: phase out of range");
-    CU(cudaSetDevice(ctx->device));
+    const int rc = pbs4d_mc_dose_phases(ctx, 1, &phase, seed, per_protons, stats, nullptr);
+    if (rc != PBS4D_OK) return rc;
     const size_t nvox = ctx->nvox();
-    PhaseLaunch& L = ctx->launches[phase];
-    CU(ctx->q[phase]->ensure(nvox * sizeof(long long)));
-    CU(ctx->dose[phase]->ensure(nvox * sizeof(float)));
-    CU(ctx->counters.ensure(sizeof(TransportCounters)));
-    CU(cudaMemsetAsync(ctx->q[phase]->p, 0, nvox * sizeof(long long), ctx->stream));
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(TransportCounters), ctx->stream));
-    float ms = 0.0f;
-    if (L.n_hist > 0) {
-        const size_t seg_bytes = L.segs.size() * sizeof(DevSegment);
-        CU(ctx->seg_dev.ensure(seg_bytes + L.segs.size() * sizeof(long long)));
-        CU(cudaMemcpyAsync(ctx->seg_dev.p, L.segs.data(), seg_bytes, cudaMemcpyHostToDevice, ctx->stream));
-        CU(cudaMemcpyAsync(ctx->seg_dev.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
-                           cudaMemcpyHostToDevice, ctx->stream));
-        cudaEvent_t e0, e1;
-        CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
-        CU(cudaEventRecord(e0, ctx->stream));
-        launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->seg_dev.as<DevSegment>(),
-                         reinterpret_cast<const long long*>(ctx->seg_dev.as<char>() + seg_bytes), (int32_t)L.segs.size(), L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
-                         ctx->counters.as<TransportCounters>(), ctx->sm_count, ctx->stream);
-        CU(cudaEventRecord(e1, ctx->stream));
-        CU(cudaGetLastError());
-        CU(cudaEventSynchronize(e1));
-        CU(cudaEventElapsedTime(&ms, e0, e1));
-        cudaEventDestroy(e0); cudaEventDestroy(e1);
-    }
-    launch_finalize_dose(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->q[phase]->as<long long>(),
-                         ctx->fixed_shift, per_protons, ctx->dose[phase]->as<float>(), ctx->stream);
-    CU(cudaGetLastError());
     if (dose_dev) CU(cudaMemcpyAsync(dose_dev, ctx->dose[phase]->p, nvox * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
     if (rho_dev)  CU(cudaMemcpyAsync(rho_dev, ctx->rho[phase]->p, nvox * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
-    TransportCounters tc{};
-    CU(cudaMemcpyAsync(&tc, ctx->counters.p, sizeof(tc), cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
-    ctx->have_dose[phase] = true;
-    if (stats) {
-        stats->histories = tc.histories; stats->steps = tc.steps;
-        stats->q_incident = tc.q_incident; stats->q_deposited = tc.q_deposited; stats->q_escaped = tc.q_escaped;
-        stats->fixed_shift = ctx->fixed_shift; stats->pad = 0; stats->kernel_ms = ms;
-        stats->pad2 = 0; stats->scoring_atomics = tc.reds;
-    }
+    if (dose_dev || rho_dev) CU(cudaStreamSynchronize(ctx->stream));
     return PBS4D_OK;
 }
 
@@ -478,7 +541,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
 
     // H2D: CT phases -> densities, DVFs
     const size_t ct_vox = (size_t)ct->nx * ct->ny * ct->nz;
-    DevBuf hu_dev;
+    DevBuf& hu_dev = ctx->host_hu;
     CU(hu_dev.ensure((size_t)n_phases * ct_vox * sizeof(int16_t)));
     std::vector<const int16_t*> hu_ptrs(n_phases);
     for (int p = 0; p < n_phases; ++p) {
@@ -488,10 +551,9 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     }
     int rc = pbs4d_set_ct_phases(ctx, n_phases, ct, hu_ptrs.data(), dose_grid, n_pts, hu_pts, rho_pts);
     if (rc != PBS4D_OK) return rc;
-    hu_dev.release();
     if (disp_host) {
         const size_t dvf_bytes = (size_t)3 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
-        DevBuf tmp;
+        DevBuf& tmp = ctx->host_dvf;
         for (int p = 0; p < n_phases; ++p) {
             if (p == ref_phase || !disp_host[p]) continue;
             CU(tmp.ensure(dvf_bytes));
@@ -509,16 +571,18 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     const auto t2 = clk::now();
 
     uint64_t run = 0;
-    for (int p = 0; p < n_phases; ++p) {
-        if (ctx->launches[p].n_hist <= 0 && p != ref_phase) continue;
-        pbs4d_mc_stats st{};
-        rc = pbs4d_mc_dose_phase(ctx, p, seed, 0.0, nullptr, nullptr, &st);
+    {
+        std::vector<int32_t> todo;
+        for (int p = 0; p < n_phases; ++p)
+            if (ctx->launches[p].n_hist > 0 || p == ref_phase) todo.push_back(p);
+        std::vector<pbs4d_mc_stats> st(todo.size());
+        rc = pbs4d_mc_dose_phases(ctx, (int32_t)todo.size(), todo.data(), seed, 0.0, st.data(), nullptr);
         if (rc != PBS4D_OK) return rc;
-        run += st.histories;
+        for (const auto& x : st) run += x.histories;
     }
     const auto t3 = clk::now();
 
-    DevBuf out;
+    DevBuf& out = ctx->host_out;
     CU(out.ensure(ctx->nvox() * sizeof(float)));
     rc = pbs4d_accumulate_subvoxel(ctx, ref_phase, nsx, nsy, nsz, nullptr, out.as<float>(), nullptr);
     if (rc != PBS4D_OK) return rc;

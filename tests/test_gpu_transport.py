@@ -172,3 +172,26 @@ def test_empty_phase_and_resampled_grid(ctx):
     assert (g[0][3] == o[0][3]).all()
     for p in (4, 5):
         check_parity(g[p], o[p], f"config3-small phase {p}")
+
+
+def test_batched_phases_equal_single_calls(ctx):
+    # pbs4d_mc_dose_phases (concurrent launches on internal streams) must give the integers of per-phase calls
+    cfg = synth.config3(div=4, n_hist=120_000)
+    hu = torch.from_numpy(cfg["hu"]).cuda()
+    ctx.set_ct_phases(cfg["ct_grid"], [hu[p] for p in range(hu.shape[0])], cfg["dose_grid"])
+    ctx.set_plan_spots(cfg["fields"], cfg["spots"])
+    deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
+    phases = sorted(set(int(x) for x in deliv["segments"]["phase"]))
+    assert len(phases) > 4
+    single = {}
+    for p in phases:
+        _, _, st = ctx.mc_dose_phase(p, cfg["seed"], want_dose=False)
+        single[p] = (ctx.get_phase_energy(p).clone(), st)
+    sts, ms = ctx.mc_dose_phases(phases, cfg["seed"])
+    assert ms > 0.0
+    for p, st in zip(phases, sts):
+        assert (ctx.get_phase_energy(p) == single[p][0]).all(), f"phase {p}"
+        for k in ("histories", "steps", "q_incident", "q_deposited", "q_escaped", "scoring_atomics"):
+            assert st[k] == single[p][1][k], (p, k)
+    with pytest.raises(RuntimeError):
+        ctx.mc_dose_phases([phases[0], phases[0]], cfg["seed"])
