@@ -49,6 +49,8 @@ def lib():
         _lib.orc_hu_to_density.restype = C.c_int
         _lib.orc_emtm_push.restype = C.c_int
         _lib.orc_emtm_finalize.restype = C.c_int
+        _lib.orc_dim_pull.restype = C.c_int
+        _lib.orc_dim_finalize.restype = C.c_int
     return _lib
 
 
@@ -204,3 +206,39 @@ def accumulate_subvoxel(grid, doses, rhos, disps, dvf_grids, ref_phase, ns_xyz):
         for k in ACCSTAT_DT.names:
             stats[k] += st[k]
     return emtm_finalize(grid, doses[ref_phase], Es, Ms, dgs), stats
+
+
+def dim_pull(ref_grid, ns_xyz, dvf_grid, disp, src_grid, dose_src):
+    """P1-P5 (Eq. 3) for one source phase.  disp = T^{R->S} on dvf_grid (reference frame).
+    Returns (D_i^S float64 on the reference grid, stats record)."""
+    disp = np.ascontiguousarray(disp, np.float32)
+    dose_src = np.ascontiguousarray(dose_src, np.float32)
+    out = np.zeros(grid_shape(ref_grid), np.float64)
+    st = np.zeros(1, ACCSTAT_DT)
+    rc = lib().orc_dim_pull(_p(ref_grid), C.c_int32(ns_xyz[0]), C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]),
+                            _p(dvf_grid), _p(disp), _p(src_grid), _p(dose_src), _p(out), _p(st))
+    if rc != 0:
+        raise ValueError(f"orc_dim_pull: error {rc}")
+    return out, st[0]
+
+
+def accumulate_dim(grid, doses, disps_pull, dvf_grids, ref_phase, ns_xyz):
+    """Whole DIM path: doses per phase on `grid`; disps_pull[p] = T^{R->S_p} displacement (None: phase not pulled)."""
+    pulled, dgs = [], []
+    stats = np.zeros(1, ACCSTAT_DT)[0]
+    for p in range(len(doses)):
+        if p == ref_phase or disps_pull[p] is None:
+            continue
+        d, st = dim_pull(grid, ns_xyz, dvf_grids[p], disps_pull[p], grid, doses[p])
+        pulled.append(d); dgs.append(dvf_grids[p])
+        for k in ACCSTAT_DT.names:
+            stats[k] += st[k]
+    n = len(pulled)
+    P = np.ascontiguousarray(np.stack(pulled), np.float64) if n else None
+    dg = np.ascontiguousarray(np.concatenate(dgs), GRID_DT) if n else None
+    out = np.zeros(grid_shape(grid), np.float32)
+    rc = lib().orc_dim_finalize(_p(grid), _p(np.ascontiguousarray(doses[ref_phase], np.float32)), C.c_int32(n), _p(P),
+                                _p(dg), _p(out))
+    if rc != 0:
+        raise ValueError(f"orc_dim_finalize: error {rc}")
+    return out, stats

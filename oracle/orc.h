@@ -107,6 +107,19 @@ int orc_emtm_push(const orc_grid* src, const float* dose, const float* rho,
 int orc_emtm_finalize(const orc_grid* ref, const float* dose_ref, int32_t n_src,
                       const int64_t* E, const int64_t* M, const orc_grid* dvf_grids, float* out);
 
+/* ---- dose-interpolation method (DIM), Eq. 3; steps P1-P5 in orc_dim.c ----
+ * Pull one source phase: dose_pulled[i] = D_i^S (double) for every reference voxel.  disp = T^{R->S} as displacements
+ * [3][z][y][x] mm on grid Dg in the REFERENCE frame; dose_src on grid S.  stats: subvoxels, dropped_outside_ref =
+ * mapped points outside the source grid, dropped_outside_dvf = subvoxel centres outside the DVF grid. */
+int orc_dim_pull(const orc_grid* R, int32_t nsx, int32_t nsy, int32_t nsz,
+                 const orc_grid* Dg, const float* disp, const orc_grid* S, const float* dose_src,
+                 double* dose_pulled, orc_acc_stats* stats);
+
+/* Eq. 2 + mask for n_src pulled phases: out = (float)(D_ref + sum_S pulled[S]) in ascending order, 0 where the voxel
+ * centre is outside any DVF's extent.  pulled: [n_src][R voxels]. */
+int orc_dim_finalize(const orc_grid* R, const float* dose_ref, int32_t n_src, const double* pulled,
+                     const orc_grid* dvf_grids, float* out);
+
 #ifdef __cplusplus
 }
 #endif
