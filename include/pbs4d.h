@@ -169,6 +169,22 @@ int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, 
                         int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
                         double* seconds);
 
+/* ---- dose-interpolation method (DIM), the paper's second accumulation method (Eq. 3; "Input
+ * options allowed the user to choose both the accumulation method and the voxel-subdivision scale n").
+ * DIMs use deformation fields of the opposite direction: T^{R->S} as displacements [3][z][y][x] (mm)
+ * at the centres of an axis-aligned grid in the REFERENCE phase frame; copied.  Requires set_ct_phases /
+ * set_density_phases first (they define the dose grid). */
+int pbs4d_set_dvf_pull(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
+                       const float* disp_dev);
+
+/* Eq. 3 for every source phase that has a T^{R->S} field to ref_phase: each reference voxel is split into
+ * nsx*nsy*nsz subvoxels, each centre is mapped to the source phase, the trilinearly interpolated source dose there
+ * (0 outside the source grid) is averaged over the subvoxels; then Eq. 2 (sum over phases in ascending order, in
+ * double) and the DVF-coverage mask.  Arguments as for accumulate_subvoxel; in stats,
+ * dropped_outside_ref counts mapped points outside the source grid, push_ms is the device time of the pull kernels. */
+int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                         const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats);
+
 /* In-run roofline probes (BASELINE.json north_star: throughput is reported "as achieved fraction of the FP32-issue,
  * L2-atomic and HBM roofline measured by in-run microbenchmarks").  Each probe launches a small kernel of its own on
  * the context's stream, times it with CUDA events (best of 3-5 after a warm-up) and writes one number to *value:

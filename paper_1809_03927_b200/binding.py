@@ -28,7 +28,8 @@ NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
 EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
            "pbs4d_mc_dose_phase", "pbs4d_mc_dose_phases", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
-           "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe"]
+           "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe",
+           "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim"]
 
 
 class PhaseLists(C.Structure):
@@ -167,6 +168,13 @@ class Context:
         self._check(self.lib.pbs4d_set_dvf(self.h, C.c_int32(src_phase), C.c_int32(ref_phase), _np(g),
                                            C.c_void_p(disp.data_ptr())))
 
+    def set_dvf_pull(self, src_phase, ref_phase, dvf_grid, disp):
+        """T^{R->S} displacement field in the reference frame (dose-interpolation method)"""
+        g = np.ascontiguousarray(dvf_grid, GRID_DT)
+        self._dev(disp, self.torch.float32)
+        self._check(self.lib.pbs4d_set_dvf_pull(self.h, C.c_int32(src_phase), C.c_int32(ref_phase), _np(g),
+                                                C.c_void_p(disp.data_ptr())))
+
     def set_plan_spots(self, fields, spots):
         f = np.ascontiguousarray(fields, FIELD_DT)
         s = np.ascontiguousarray(spots, SPOT_DT)
@@ -227,6 +235,18 @@ class Context:
         self._check(self.lib.pbs4d_accumulate_subvoxel(self.h, C.c_int32(ref_phase), C.c_int32(ns_xyz[0]),
                                                        C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), ptrs,
                                                        C.c_void_p(out.data_ptr()), C.byref(st)))
+        return out, st.as_dict()
+
+    def accumulate_dim(self, ref_phase, ns_xyz, phase_doses=None):
+        t = self.torch
+        out = t.empty(self.dose_shape, dtype=t.float32, device=self.device)
+        ptrs = None
+        if phase_doses is not None:
+            ptrs = _ptr_array([None if d is None else self._dev(d, t.float32) for d in phase_doses])
+        st = AccStats()
+        self._check(self.lib.pbs4d_accumulate_dim(self.h, C.c_int32(ref_phase), C.c_int32(ns_xyz[0]),
+                                                  C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), ptrs,
+                                                  C.c_void_p(out.data_ptr()), C.byref(st)))
         return out, st.as_dict()
 
     def get_accumulators(self, src_phase):

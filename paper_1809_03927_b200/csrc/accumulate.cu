@@ -266,6 +266,148 @@ emtm_finalize_kernel(const __grid_constant__ FinalizeParams P)
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Dose-interpolation method (DIM, Eq. 3): pull.  One thread per reference voxel loops over its
+// nsx*nsy*nsz subvoxel centres r_ik: displacement T^{R->S}(r_ik) by trilinear interpolation of the (float4) DVF,
+// q = r + u, trilinear dose of the source phase at q (clamp-to-edge inside the source grid's voxel extent, 0
+// outside), sum in double in (c, b, a) order, D_i^S = sum / n^3, added to a double accumulator that was initialised
+// with D_i^R (Eq. 2: phases are added in ascending order, one launch per source phase on one stream).
+// No atomics: every reference voxel is owned by one thread.
+// ------------------------------------------------------------------------------------------------------------------
+struct PullParams {
+    pbs4d_grid ref, dvf, src;
+    const float4* __restrict__ U;            // T^{R->S}, interleaved, on grid dvf (reference frame)
+    const float* __restrict__ dose;          // source-phase dose on grid src
+    double* acc;                             // [ref voxels]
+    int nsx, nsy, nsz;
+    AccCounters* counters;
+};
+
+struct Cell { int i0, d1; float w; bool ok; };
+__device__ __forceinline__ Cell cell_of(float p, float o, float h, int n)
+{
+    Cell c;
+    float g = __fsub_rn(__fdiv_rn(__fsub_rn(p, o), h), 0.5f);
+    c.ok = (g >= -0.5f) && (g < __fsub_rn((float)n, 0.5f));
+    g = fminf(fmaxf(g, 0.0f), (float)(n - 1));
+    int k = (int)floorf(g);
+    k = max(min(k, n - 2), 0);
+    c.i0 = k;
+    c.d1 = min(k + 1, n - 1) - k;
+    c.w  = __fsub_rn(g, (float)k);
+    return c;
+}
+
+__global__ void __launch_bounds__(kTileX * kTileY)
+dim_pull_kernel(const __grid_constant__ PullParams P)
+{
+    extern __shared__ AxisEntry s_map[];
+    AxisEntry* sx = s_map;
+    AxisEntry* sy = sx + kTileX * P.nsx;
+    AxisEntry* sz = sy + kTileY * P.nsy;
+    const int tid = threadIdx.y * kTileX + threadIdx.x;
+    const int i = blockIdx.x * kTileX + threadIdx.x;
+    const int j = blockIdx.y * kTileY + threadIdx.y;
+    const int k = blockIdx.z;
+    const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy;
+    for (int e = tid; e < n_x + n_y + P.nsz; e += kTileX * kTileY) {
+        if (e < n_x)
+            s_map[e] = axis_map(P.ref.ox, P.ref.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
+                                P.dvf.ox, P.dvf.hx, P.dvf.nx);
+        else if (e < n_x + n_y)
+            s_map[e] = axis_map(P.ref.oy, P.ref.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
+                                P.dvf.oy, P.dvf.hy, P.dvf.ny);
+        else
+            s_map[e] = axis_map(P.ref.oz, P.ref.hz, k, e - n_x - n_y, P.nsz, P.dvf.oz, P.dvf.hz, P.dvf.nz);
+    }
+    __syncthreads();
+
+    unsigned n_src = 0, n_dvf = 0;
+    if (i < P.ref.nx && j < P.ref.ny) {
+        const int nsx = P.nsx, nsy = P.nsy, nsz = P.nsz;
+        const int dnx = P.dvf.nx, dny = P.dvf.ny;
+        const int dx1 = dnx > 1 ? 1 : 0;
+        const int snx = P.src.nx, sny = P.src.ny, snz = P.src.nz;
+        const float sox = P.src.ox, soy = P.src.oy, soz = P.src.oz, shx = P.src.hx, shy = P.src.hy, shz = P.src.hz;
+        const AxisEntry* sxl = sx + threadIdx.x;
+        const AxisEntry* syl = sy + threadIdx.y * nsy;
+        double sum = 0.0;
+        for (int c = 0; c < nsz; ++c) {
+            const AxisEntry mz = sz[c];
+            for (int b = 0; b < nsy; ++b) {
+                const AxisEntry my = syl[b];
+                const int r00 = (mz.i0 * dny + my.i0) * dnx;
+                const int sy1 = (my.flags & 1) * dnx, sz1 = (mz.flags & 1) * dny * dnx;
+                const float4* __restrict__ p00 = P.U + r00;
+                const float4* __restrict__ p01 = p00 + sy1;
+                const float4* __restrict__ p10 = p00 + sz1;
+                const float4* __restrict__ p11 = p10 + sy1;
+                const bool ok_zy = (mz.flags & my.flags & 2) != 0;
+                for (int a = 0; a < nsx; ++a) {
+                    const AxisEntry mx = sxl[a * kTileX];
+                    if (!(ok_zy && (mx.flags & 2))) { n_dvf += 1; continue; }
+                    const int x0 = mx.i0;
+                    const float4 a000 = __ldg(p00 + x0), a001 = __ldg(p00 + x0 + dx1);
+                    const float4 a010 = __ldg(p01 + x0), a011 = __ldg(p01 + x0 + dx1);
+                    const float4 a100 = __ldg(p10 + x0), a101 = __ldg(p10 + x0 + dx1);
+                    const float4 a110 = __ldg(p11 + x0), a111 = __ldg(p11 + x0 + dx1);
+#define PBS4D_TRILERP(cmp) lerp_rn(lerp_rn(lerp_rn(a000.cmp, a001.cmp, mx.w), lerp_rn(a010.cmp, a011.cmp, mx.w), my.w), \
+                                   lerp_rn(lerp_rn(a100.cmp, a101.cmp, mx.w), lerp_rn(a110.cmp, a111.cmp, mx.w), my.w), mz.w)
+                    const float qx = __fadd_rn(mx.p, PBS4D_TRILERP(x));
+                    const float qy = __fadd_rn(my.p, PBS4D_TRILERP(y));
+                    const float qz = __fadd_rn(mz.p, PBS4D_TRILERP(z));
+#undef PBS4D_TRILERP
+                    const Cell cx = cell_of(qx, sox, shx, snx), cy = cell_of(qy, soy, shy, sny),
+                               cz = cell_of(qz, soz, shz, snz);
+                    if (!(cx.ok && cy.ok && cz.ok)) { n_src += 1; continue; }
+                    const float* __restrict__ d00 = P.dose + ((size_t)cz.i0 * sny + cy.i0) * snx + cx.i0;
+                    const float* __restrict__ d01 = d00 + cy.d1 * snx;
+                    const float* __restrict__ d10 = d00 + (size_t)cz.d1 * sny * snx;
+                    const float* __restrict__ d11 = d10 + cy.d1 * snx;
+                    const float c00 = lerp_rn(__ldg(d00), __ldg(d00 + cx.d1), cx.w);
+                    const float c01 = lerp_rn(__ldg(d01), __ldg(d01 + cx.d1), cx.w);
+                    const float c10 = lerp_rn(__ldg(d10), __ldg(d10 + cx.d1), cx.w);
+                    const float c11 = lerp_rn(__ldg(d11), __ldg(d11 + cx.d1), cx.w);
+                    const float val = lerp_rn(lerp_rn(c00, c01, cy.w), lerp_rn(c10, c11, cy.w), cz.w);
+                    sum = __dadd_rn(sum, (double)val);
+                }
+            }
+        }
+        const size_t v = ((size_t)k * P.ref.ny + j) * P.ref.nx + i;
+        const double n3 = __dmul_rn(__dmul_rn((double)nsx, (double)nsy), (double)nsz);
+        P.acc[v] = __dadd_rn(P.acc[v], __ddiv_rn(sum, n3));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        n_src += __shfl_xor_sync(0xffffffffu, n_src, off);
+        n_dvf += __shfl_xor_sync(0xffffffffu, n_dvf, off);
+    }
+    if (threadIdx.x == 0) {
+        if (n_src) atomicAdd(&P.counters->dropped_ref, (unsigned long long)n_src);
+        if (n_dvf) atomicAdd(&P.counters->dropped_dvf, (unsigned long long)n_dvf);
+    }
+}
+
+__global__ void dim_init_kernel(size_t n, const float* __restrict__ dose_ref, double* __restrict__ acc)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) acc[i] = (double)dose_ref[i];
+}
+
+__global__ void __launch_bounds__(128)
+dim_final_kernel(pbs4d_grid ref, const double* __restrict__ acc, const unsigned char* __restrict__ flags,
+                 float* __restrict__ out)
+{
+    const int row = blockIdx.x;
+    const int nx = ref.nx, ny = ref.ny;
+    const int j = row % ny, k = row / ny;
+    const bool row_ok = flags[nx + j] && flags[nx + ny + k];
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
+    if (i >= nx) return;
+    const size_t v = (size_t)row * nx + i;
+    out[v] = (row_ok && flags[i]) ? (float)acc[v] : 0.0f;
+}
+
 }  // namespace
 
 void launch_dvf_interleave(const pbs4d_grid& g, const float* disp_planar, float* out4, cudaStream_t st)
@@ -310,6 +452,36 @@ void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_sr
     dim3 g(ref.ny * ref.nz, (per_row + 127) / 128);
     if (pair) emtm_finalize_kernel<true><<<g, 128, 0, st>>>(P);
     else      emtm_finalize_kernel<false><<<g, 128, 0, st>>>(P);
+}
+
+void launch_dim_init(const pbs4d_grid& ref, const float* dose_ref, double* acc, cudaStream_t st)
+{
+    const size_t n = (size_t)ref.nx * ref.ny * ref.nz;
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 16);
+    dim_init_kernel<<<blocks, 256, 0, st>>>(n, dose_ref, acc);
+}
+
+void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs4d_grid& dvf_grid, const float* disp4,
+                     const pbs4d_grid& src, const float* dose_src, double* acc, AccCounters* counters, cudaStream_t st)
+{
+    PullParams P;
+    P.ref = ref; P.dvf = dvf_grid; P.src = src; P.U = reinterpret_cast<const float4*>(disp4); P.dose = dose_src;
+    P.acc = acc; P.nsx = nsx; P.nsy = nsy; P.nsz = nsz; P.counters = counters;
+    dim3 b(kTileX, kTileY, 1), g((ref.nx + kTileX - 1) / kTileX, (ref.ny + kTileY - 1) / kTileY, ref.nz);
+    const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + nsz) * sizeof(AxisEntry);
+    dim_pull_kernel<<<g, b, smem, st>>>(P);
+}
+
+void launch_dim_final(const pbs4d_grid& ref, int n_src, const pbs4d_grid* dvf_grids_host, const double* acc,
+                      unsigned char* flags_dev, float* out, cudaStream_t st)
+{
+    CoverParams C;
+    C.ref = ref; C.n_src = n_src; C.flags = flags_dev;
+    for (int s = 0; s < n_src && s < kMaxSrc; ++s) C.dvf[s] = dvf_grids_host[s];
+    const int n_axis = ref.nx + ref.ny + ref.nz;
+    emtm_cover_kernel<<<(n_axis + 127) / 128, 128, 0, st>>>(C);
+    dim3 g(ref.ny * ref.nz, (ref.nx + 127) / 128);
+    dim_final_kernel<<<g, 128, 0, st>>>(ref, acc, flags_dev, out);
 }
 
 }  // namespace pbs4d

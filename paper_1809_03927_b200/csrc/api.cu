@@ -56,7 +56,9 @@ struct pbs4d_ctx {
 
     // DVFs (a2)
     struct Dvf { bool set = false; int32_t ref = -1; pbs4d_grid grid{}; std::unique_ptr<DevBuf> disp; };
-    std::vector<Dvf> dvf;                                // [src phase]
+    std::vector<Dvf> dvf;                                // [src phase] T^{S->R} (push, EMTM)
+    std::vector<Dvf> dvf_pull;                           // [src phase] T^{R->S} (pull, DIM)
+    DevBuf dim_acc;                                      // double accumulator of the DIM [ref voxels]
 
     // plan (a2) and delivery (a3)
     std::vector<pbs4d_field> fields;
@@ -122,6 +124,8 @@ void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
     fit(ctx->rho); fit(ctx->q); fit(ctx->dose); fit(ctx->accE); fit(ctx->accM);
     ctx->dvf.resize(n_phases);
     for (auto& d : ctx->dvf) { d.set = false; d.ref = -1; }
+    ctx->dvf_pull.resize(n_phases);
+    for (auto& d : ctx->dvf_pull) { d.set = false; d.ref = -1; }
     ctx->have_dose.assign(n_phases, false);
     ctx->have_acc.assign(n_phases, false);
     ctx->have_density = false;
@@ -208,16 +212,16 @@ int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid*
     return PBS4D_OK;
 }
 
-int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
-                  const float* disp_dev)
+static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const char* who, int32_t src_phase,
+                     int32_t ref_phase, const pbs4d_grid* dvf_grid, const float* disp_dev)
 {
     if (!ctx) return PBS4D_ERR_ARG;
-    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "set_dvf: call set_ct_phases/set_density_phases first");
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, std::string(who) + ": call set_ct_phases/set_density_phases first");
     if (src_phase < 0 || src_phase >= ctx->n_phases || ref_phase < 0 || ref_phase >= ctx->n_phases ||
         src_phase == ref_phase || !grid_ok(dvf_grid) || !disp_dev)
-        return fail(ctx, PBS4D_ERR_ARG, "set_dvf: bad argument");
+        return fail(ctx, PBS4D_ERR_ARG, std::string(who) + ": bad argument");
     CU(cudaSetDevice(ctx->device));
-    auto& d = ctx->dvf[src_phase];
+    auto& d = table[src_phase];
     if (!d.disp) d.disp.reset(new DevBuf);
     const size_t bytes = (size_t)4 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
     CU(d.disp->ensure(bytes));
@@ -226,6 +230,20 @@ int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pb
     CU(cudaStreamSynchronize(ctx->stream));
     d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
     return PBS4D_OK;
+}
+
+int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
+                  const float* disp_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    return store_dvf(ctx, ctx->dvf, "set_dvf", src_phase, ref_phase, dvf_grid, disp_dev);
+}
+
+int pbs4d_set_dvf_pull(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
+                       const float* disp_dev)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    return store_dvf(ctx, ctx->dvf_pull, "set_dvf_pull", src_phase, ref_phase, dvf_grid, disp_dev);
 }
 
 int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fields,
@@ -610,5 +628,59 @@ extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value)
         case PBS4D_PROBE_RED_HOT:    CU(probe_l2_atomic(ctx->sm_count, 1, ctx->stream, value)); break;
         default:                     CU(probe_hbm_copy(ctx->sm_count, ctx->stream, value)); break;
     }
+    return PBS4D_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// dose-interpolation accumulation (DIM, Eq. 3): pull every source phase with a T^{R->S} field
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                                    const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_dim: no grid (set_ct_phases/set_density_phases)");
+    if (ref_phase < 0 || ref_phase >= ctx->n_phases || nsx < 1 || nsy < 1 || nsz < 1 || nsx > 64 || nsy > 64 ||
+        nsz > 64 || !dose4d_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "accumulate_dim: bad argument");
+    auto dose_of = [&](int p) -> const float* {
+        if (phase_dose_dev) return phase_dose_dev[p];
+        return ctx->have_dose[p] ? ctx->dose[p]->as<float>() : nullptr;
+    };
+    if (!dose_of(ref_phase)) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_dim: no dose for the reference phase");
+    std::vector<int> src;
+    for (int p = 0; p < ctx->n_phases; ++p)
+        if (p != ref_phase && ctx->dvf_pull[p].set && ctx->dvf_pull[p].ref == ref_phase && dose_of(p)) src.push_back(p);
+    CU(cudaSetDevice(ctx->device));
+    const size_t nvox = ctx->nvox();
+    CU(ctx->acc_counters.ensure(sizeof(AccCounters)));
+    CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
+    CU(ctx->dim_acc.ensure(nvox * sizeof(double)));
+    CU(ctx->cover_flags.ensure((size_t)ctx->dose_grid.nx + ctx->dose_grid.ny + ctx->dose_grid.nz));
+    cudaEvent_t e0, e1, e2;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1)); CU(cudaEventCreate(&e2));
+    launch_dim_init(ctx->dose_grid, dose_of(ref_phase), ctx->dim_acc.as<double>(), ctx->stream);
+    CU(cudaEventRecord(e0, ctx->stream));
+    std::vector<pbs4d_grid> dg;
+    for (int p : src) {                                  // ascending phase order: Eq. 2 is summed in this order
+        launch_dim_pull(ctx->dose_grid, nsx, nsy, nsz, ctx->dvf_pull[p].grid, ctx->dvf_pull[p].disp->as<float>(),
+                        ctx->dose_grid, dose_of(p), ctx->dim_acc.as<double>(), ctx->acc_counters.as<AccCounters>(),
+                        ctx->stream);
+        dg.push_back(ctx->dvf_pull[p].grid);
+    }
+    CU(cudaEventRecord(e1, ctx->stream));
+    launch_dim_final(ctx->dose_grid, (int)src.size(), dg.data(), ctx->dim_acc.as<double>(),
+                     ctx->cover_flags.as<unsigned char>(), dose4d_dev, ctx->stream);
+    CU(cudaEventRecord(e2, ctx->stream));
+    CU(cudaGetLastError());
+    AccCounters ac{};
+    CU(cudaMemcpyAsync(&ac, ctx->acc_counters.p, sizeof(ac), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (stats) {
+        stats->subvoxels = (uint64_t)src.size() * nvox * nsx * nsy * nsz;
+        stats->dropped_outside_ref = ac.dropped_ref; stats->dropped_outside_dvf = ac.dropped_dvf;
+        cudaEventElapsedTime(&stats->push_ms, e0, e1);
+        cudaEventElapsedTime(&stats->finalize_ms, e1, e2);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
     return PBS4D_OK;
 }

@@ -61,6 +61,13 @@ void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_sr
                           const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev,
                           unsigned char* flags_dev /*[nx+ny+nz] scratch*/, float* out, cudaStream_t st);
 
+// ---- dose-interpolation method (accumulate.cu) ----
+void launch_dim_init(const pbs4d_grid& ref, const float* dose_ref, double* acc, cudaStream_t st);
+void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs4d_grid& dvf_grid, const float* disp4,
+                     const pbs4d_grid& src, const float* dose_src, double* acc, AccCounters* counters, cudaStream_t st);
+void launch_dim_final(const pbs4d_grid& ref, int n_src, const pbs4d_grid* dvf_grids_host, const double* acc,
+                      unsigned char* flags_dev, float* out, cudaStream_t st);
+
 // ---- in-run roofline probes (roofline.cu) ----
 #ifdef __CUDACC__
 cudaError_t probe_fp32_issue(int sm_count, cudaStream_t st, double* lane_inst_per_s);
