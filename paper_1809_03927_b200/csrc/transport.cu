@@ -6,13 +6,15 @@
 //
 // Layout of the computation (B200-first, not the paper's Titan-X design).  The kernel is bound by instruction
 // issue and by the XU (MUFU/conversion) pipe, never by HBM, so everything below is about instructions per step:
-//  * persistent warps; a lane whose history ends takes the next history index from a global counter (one
-//    warp-aggregated atomicAdd), so all lanes stay busy until the launch runs out of histories.  The Philox counter
-//    is (step, history), never the lane, so any lane/history assignment gives the same integers;
-//  * the step loop is warp-uniform (refill phase, then one predicated step for every live lane): the warp
-//    reconverges every iteration;
+//  * persistent warps (4 CTAs x 256 threads per SM, 64 registers).  Every warp keeps a pool of 32 pre-sampled
+//    histories in shared memory: when it is empty the whole warp takes 32 history indices from a global counter
+//    (one atomicAdd) and samples them together, and a lane whose history ends pops the next entry.  The Philox
+//    counter is (step, history), never the lane, so any lane/history assignment gives the same integers;
+//  * the step loop is warp-uniform (refill phase, then one predicated, branch-free step for every live lane): the
+//    warp reconverges every iteration;
 //  * S(E), 2 % of the CSDA range, the Bohr variance and the Highland theta0^2 come from ONE float4 table in shared
 //    memory, indexed by integer operations on the bit pattern of E (no logarithm), linear in E inside an interval;
+//    the values at the midpoint energy are read off the same pair of nodes (one lookup per step);
 //  * one reciprocal per step for the voxel-face distance (the nearest face is found by cross-multiplication),
 //    1/density cached per voxel visit, Gaussian factors folded under one square root each, small-angle polynomial
 //    for the polar deflection, uniform floats built with bit operations: 9 MUFU per step instead of ~27;
