@@ -79,6 +79,7 @@ struct pbs4d_ctx {
     DevBuf counters;
     std::vector<std::unique_ptr<DevBuf>> seg_phase;      // [phase] launch table (DevSegment[] | seg_begin[])
     std::vector<cudaStream_t> aux;                       // auxiliary streams for concurrent phase launches
+    cudaStream_t copy_stream = nullptr;                  // uploads that overlap compute (run_plan_host)
 
     // accumulation state (a8-a9)
     std::vector<std::unique_ptr<DevBuf>> accE, accM;     // [phase]
@@ -158,6 +159,7 @@ void pbs4d_destroy(pbs4d_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (auto st : ctx->aux) if (st) cudaStreamDestroy(st);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
     delete ctx;
 }
 
@@ -569,16 +571,31 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     }
     int rc = pbs4d_set_ct_phases(ctx, n_phases, ct, hu_ptrs.data(), dose_grid, n_pts, hu_pts, rho_pts);
     if (rc != PBS4D_OK) return rc;
+    // DVFs are not needed before the accumulation: their upload (the bulk of the host->device bytes) and re-layout
+    // run on a copy stream underneath the delivery simulation and the transport kernels
+    struct CopyGuard {                                   // an early error return must not leave copies from the
+        cudaStream_t st = nullptr; cudaEvent_t ev = nullptr;   // caller's host buffers in flight
+        ~CopyGuard() { if (ev) { cudaStreamSynchronize(st); cudaEventDestroy(ev); } }
+    } guard;
+    cudaEvent_t& dvf_ready = guard.ev;
     if (disp_host) {
-        const size_t dvf_bytes = (size_t)3 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
+        if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        const size_t dvf_vox = (size_t)dvf_grid->nx * dvf_grid->ny * dvf_grid->nz;
         DevBuf& tmp = ctx->host_dvf;
+        CU(tmp.ensure(3 * dvf_vox * sizeof(float)));
         for (int p = 0; p < n_phases; ++p) {
             if (p == ref_phase || !disp_host[p]) continue;
-            CU(tmp.ensure(dvf_bytes));
-            CU(cudaMemcpyAsync(tmp.p, disp_host[p], dvf_bytes, cudaMemcpyHostToDevice, ctx->stream));
-            rc = pbs4d_set_dvf(ctx, p, ref_phase, dvf_grid, tmp.as<float>());
-            if (rc != PBS4D_OK) return rc;
+            auto& d = ctx->dvf[p];
+            if (!d.disp) d.disp.reset(new DevBuf);
+            CU(d.disp->ensure(4 * dvf_vox * sizeof(float)));
+            CU(cudaMemcpyAsync(tmp.p, disp_host[p], 3 * dvf_vox * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
+            launch_dvf_interleave(*dvf_grid, tmp.as<float>(), d.disp->as<float>(), ctx->copy_stream);
+            d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
         }
+        CU(cudaGetLastError());
+        guard.st = ctx->copy_stream;
+        CU(cudaEventCreateWithFlags(&dvf_ready, cudaEventDisableTiming));
+        CU(cudaEventRecord(dvf_ready, ctx->copy_stream));
     }
     const auto t1 = clk::now();
 
@@ -602,6 +619,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
 
     DevBuf& out = ctx->host_out;
     CU(out.ensure(ctx->nvox() * sizeof(float)));
+    if (dvf_ready) CU(cudaStreamWaitEvent(ctx->stream, dvf_ready, 0));
     rc = pbs4d_accumulate_subvoxel(ctx, ref_phase, nsx, nsy, nsz, nullptr, out.as<float>(), nullptr);
     if (rc != PBS4D_OK) return rc;
     CU(cudaMemcpyAsync(dose4d_host, out.p, ctx->nvox() * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
