@@ -44,6 +44,7 @@ def lib():
         _lib.orc_theta0_sq_per_t.argtypes = [C.c_double]
         _lib.orc_simulate_delivery.restype = C.c_int64
         _lib.orc_fixed_shift.restype = C.c_int32
+        _lib.orc_simulate_delivery_ext.restype = C.c_int64
         _lib.orc_transport.restype = C.c_int
         _lib.orc_finalize_dose.restype = None
         _lib.orc_hu_to_density.restype = C.c_int
@@ -242,3 +243,31 @@ def accumulate_dim(grid, doses, disps_pull, dvf_grids, ref_phase, ns_xyz):
     if rc != 0:
         raise ValueError(f"orc_dim_finalize: error {rc}")
     return out, stats
+
+
+class DeliveryExt(C.Structure):
+    """orc_delivery_ext (orc.h): extended delivery model, all zero / None = base model"""
+    _fields_ = [("n_cycles", C.c_int32), ("cycle_period_ns", C.c_void_p), ("discard_ns", C.c_int64),
+                ("spill_protons_max", C.c_int64), ("flat_top_ns", C.c_int64), ("spot_switch_fixed_ns", C.c_int64),
+                ("n_layer_switch", C.c_int32), ("layer_switch_ns", C.c_void_p), ("max_protons_per_paint", C.c_int64)]
+
+
+def simulate_delivery_ext(fields, spots, prm, total_histories, cycle_period_ns=None, discard_ns=0, spill_protons_max=0,
+                          flat_top_ns=0, spot_switch_fixed_ns=0, layer_switch_ns=None, max_protons_per_paint=0):
+    """E1-E5 + D6-D7.  Returns (segments, per-field end time [ns], dropped protons, synchrotron fills)."""
+    f = np.ascontiguousarray(fields, FIELD_DT); s = np.ascontiguousarray(spots, SPOT_DT)
+    p = np.ascontiguousarray(prm, DELIV_DT)
+    cyc = None if cycle_period_ns is None else np.ascontiguousarray(cycle_period_ns, np.int64)
+    lsw = None if layer_switch_ns is None else np.ascontiguousarray(layer_switch_ns, np.int64)
+    x = DeliveryExt(0 if cyc is None else len(cyc), None if cyc is None else cyc.ctypes.data, int(discard_ns),
+                    int(spill_protons_max), int(flat_top_ns), int(spot_switch_fixed_ns),
+                    0 if lsw is None else len(lsw), None if lsw is None else lsw.ctypes.data, int(max_protons_per_paint))
+    args = [C.c_int32(len(f)), _p(f), C.c_int64(len(s)), _p(s), _p(p), C.byref(x), C.c_uint64(int(total_histories))]
+    n = lib().orc_simulate_delivery_ext(*args, None, C.c_int64(0), None, None, None)
+    if n < 0:
+        raise ValueError(f"orc_simulate_delivery_ext: error {n}")
+    segs = np.zeros(n, SEG_DT); tt = np.zeros(len(f), np.int64)
+    dropped = C.c_int64(0); fills = C.c_int64(0)
+    n2 = lib().orc_simulate_delivery_ext(*args, _p(segs), C.c_int64(n), _p(tt), C.byref(dropped), C.byref(fills))
+    assert n2 == n
+    return segs, tt, int(dropped.value), int(fills.value)

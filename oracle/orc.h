@@ -57,6 +57,22 @@ int64_t orc_simulate_delivery(int32_t n_fields, const orc_field* fields, int64_t
                               orc_segment* segs, int64_t max_segs, int64_t* total_time_ns,
                               int64_t* dropped_protons);
 
+/* Extended delivery model (steps E1-E5 in orc_delivery.c): all zero / NULL = base model. */
+typedef struct {
+    int32_t n_cycles; const int64_t* cycle_period_ns;   /* irregular breathing: period of cycle c (last one repeats) */
+    int64_t discard_ns;                                 /* beam discarded when extraction (re)starts (70 ms) */
+    int64_t spill_protons_max;                          /* charge capacity of one synchrotron fill; 0 = unlimited */
+    int64_t flat_top_ns;                                /* flat-top / extraction time limit of a fill; 0 = unlimited */
+    int64_t spot_switch_fixed_ns;                       /* fixed prepare/verify part of the spot-switch time */
+    int32_t n_layer_switch; const int64_t* layer_switch_ns;   /* energy-dependent reset time per layer id */
+    int64_t max_protons_per_paint;                      /* iso-layered repainting: max protons per spot delivery */
+} orc_delivery_ext;
+
+int64_t orc_simulate_delivery_ext(int32_t n_fields, const orc_field* fields, int64_t n_spots, const orc_spot* spots,
+                                  const orc_delivery_params* prm, const orc_delivery_ext* ext, uint64_t total_histories,
+                                  orc_segment* segs, int64_t max_segs, int64_t* total_time_ns,
+                                  int64_t* dropped_protons, int64_t* n_fills);
+
 /* ---- transport (T1-T12) ---- */
 #define ORC_NO_MCS       1u   /* pin switch: no Highland deflection        */
 #define ORC_NO_STRAGGLE  2u   /* pin switch: no Bohr straggling            */
