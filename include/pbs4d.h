@@ -52,6 +52,26 @@ typedef struct {
     uint32_t gate_mask;            /* bit p set = beam allowed in phase p (gating)     */
 } pbs4d_delivery_params;
 
+/* Extended delivery model: the synchrotron behaviour the paper describes beyond the constants of BASELINE.json's
+ * configs (Sec. 2.B; App. A).  The paper takes its values from its Ref. 45, which is
+ * not available: every value is an input, and the sampled breathing periods (t_ph ~ N(mu, sigma)/N) are
+ * passed in rather than drawn inside.  All zero / NULL = the base model of pbs4d_delivery_params. */
+typedef struct {
+    int32_t n_cycles; const int64_t* cycle_period_ns;  /* irregular breathing: period of breathing cycle c, ns; the
+                                                          last entry repeats; NULL: period_ns for every cycle        */
+    int64_t discard_ns;             /* beam discarded whenever extraction (re)starts: after every synchrotron reset and
+                                       after every wait for gate-on (70 ms); must be < one phase        */
+    int64_t spill_protons_max;      /* charge capacity of one synchrotron fill (~2 nC); 0 = unlimited   */
+    int64_t flat_top_ns;            /* flat-top / extraction time limit of a fill, counted from the end of the reset
+                                       (~8 s); 0 = unlimited; must exceed discard_ns + longest period  */
+    int64_t spot_switch_fixed_ns;   /* fixed prepare/verify part of the spot-switch time               */
+    int32_t n_layer_switch; const int64_t* layer_switch_ns;   /* energy-dependent reset ("layer-switch") time per layer
+                                       id; NULL or id out of range: layer_switch_ns of the base struct */
+    int64_t max_protons_per_paint;  /* iso-layered repainting with a maximum MU per spot delivery: every
+                                       painting delivers at most this many protons of each spot until none is left;
+                                       0: the base N x repainting                                                      */
+} pbs4d_delivery_ext;
+
 /* One entry of the sub-plans after history allocation. */
 typedef struct {
     int32_t field, phase, spot, pad;
@@ -129,6 +149,16 @@ int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field* fields, in
                                  const pbs4d_spot* spots, const pbs4d_delivery_params* prm, uint64_t total_histories,
                                  pbs4d_segment* segs_out, int64_t max_segs, int64_t* n_segs_out,
                                  int64_t* field_time_ns, int64_t* dropped_protons, int32_t* fixed_shift);
+
+/* The same with the extended model; *n_fills (optional) receives the number of synchrotron fills of all fields. */
+int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
+                                uint64_t total_histories, pbs4d_phase_lists* out, int64_t* n_fills);
+int pbs4d_simulate_delivery_ext_host(int32_t n_fields, const pbs4d_field* fields, int64_t n_spots,
+                                     const pbs4d_spot* spots, const pbs4d_delivery_params* prm,
+                                     const pbs4d_delivery_ext* ext, uint64_t total_histories,
+                                     pbs4d_segment* segs_out, int64_t max_segs, int64_t* n_segs_out,
+                                     int64_t* field_time_ns, int64_t* dropped_protons, int32_t* fixed_shift,
+                                     int64_t* n_fills);
 
 /* a4-a7: Monte Carlo transport of all segments of `phase` on that phase's density grid.
  * dose_dev (optional) receives fp32 Gy [z][y][x] on the dose grid for the delivered protons (divided by

@@ -200,7 +200,8 @@ int64_t orc_simulate_delivery_ext(int32_t n_fields, const orc_field* fields, int
     for (int32_t f = 0; f < n_fields; ++f) {
         int64_t t = 0;
         cycle_cursor cur = { 0, 0 };
-        const int64_t off = (int64_t)fields[f].start_phase * (period_of(prm, x, 0) / P);      /* E1 */
+        int32_t sp0 = fields[f].start_phase % P; if (sp0 < 0) sp0 += P;     /* phases are counted modulo N (B2) */
+        const int64_t off = (int64_t)sp0 * (period_of(prm, x, 0) / P);                      /* E1 */
         int first_layer = 1;
         int64_t s = 0;
         while (s < n_spots) {

@@ -29,12 +29,30 @@ EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_ph
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
            "pbs4d_mc_dose_phase", "pbs4d_mc_dose_phases", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
            "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe",
-           "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim"]
+           "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim", "pbs4d_simulate_delivery_ext", "pbs4d_simulate_delivery_ext_host"]
 
 
 class PhaseLists(C.Structure):
     _fields_ = [("n_segments", C.c_int64), ("segments", C.c_void_p), ("n_fields", C.c_int32),
                 ("field_time_ns", C.POINTER(C.c_int64)), ("dropped_protons", C.c_int64), ("fixed_shift", C.c_int32)]
+
+
+class DeliveryExt(C.Structure):
+    """pbs4d_delivery_ext: extended delivery model (all zero / None = base model)"""
+    _fields_ = [("n_cycles", C.c_int32), ("cycle_period_ns", C.c_void_p), ("discard_ns", C.c_int64),
+                ("spill_protons_max", C.c_int64), ("flat_top_ns", C.c_int64), ("spot_switch_fixed_ns", C.c_int64),
+                ("n_layer_switch", C.c_int32), ("layer_switch_ns", C.c_void_p), ("max_protons_per_paint", C.c_int64)]
+
+
+def make_delivery_ext(cycle_period_ns=None, discard_ns=0, spill_protons_max=0, flat_top_ns=0, spot_switch_fixed_ns=0,
+                      layer_switch_ns=None, max_protons_per_paint=0):
+    """-> (DeliveryExt, keepalive arrays); marshalling only"""
+    cyc = None if cycle_period_ns is None else np.ascontiguousarray(cycle_period_ns, np.int64)
+    lsw = None if layer_switch_ns is None else np.ascontiguousarray(layer_switch_ns, np.int64)
+    x = DeliveryExt(0 if cyc is None else len(cyc), None if cyc is None else cyc.ctypes.data, int(discard_ns),
+                    int(spill_protons_max), int(flat_top_ns), int(spot_switch_fixed_ns),
+                    0 if lsw is None else len(lsw), None if lsw is None else lsw.ctypes.data, int(max_protons_per_paint))
+    return x, (cyc, lsw)
 
 
 class McStats(C.Structure):
@@ -106,6 +124,29 @@ def simulate_delivery_host(fields, spots, prm, total_histories):
     if rc != 0:
         raise RuntimeError(f"pbs4d_simulate_delivery_host: error {rc}")
     return dict(segments=segs, field_time_ns=times, dropped_protons=int(dropped.value), fixed_shift=int(shift.value))
+
+
+def simulate_delivery_ext_host(fields, spots, prm, total_histories, **ext_kw):
+    """Device-free entry of the extended delivery model (pbs4d_simulate_delivery_ext_host)."""
+    lib = load()
+    f = np.ascontiguousarray(fields, FIELD_DT)
+    s = np.ascontiguousarray(spots, SPOT_DT)
+    p = np.ascontiguousarray(prm, DELIV_DT)
+    x, keep = make_delivery_ext(**ext_kw)
+    n = C.c_int64(0)
+    args = [C.c_int32(len(f)), _np(f), C.c_int64(len(s)), _np(s), _np(p), C.byref(x), C.c_uint64(int(total_histories))]
+    rc = lib.pbs4d_simulate_delivery_ext_host(*args, None, C.c_int64(0), C.byref(n), None, None, None, None)
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_simulate_delivery_ext_host: error {rc}")
+    segs = np.zeros(n.value, SEG_DT)
+    times = np.zeros(len(f), np.int64)
+    dropped = C.c_int64(0); shift = C.c_int32(0); fills = C.c_int64(0)
+    rc = lib.pbs4d_simulate_delivery_ext_host(*args, _np(segs), C.c_int64(n.value), C.byref(n), _np(times),
+                                              C.byref(dropped), C.byref(shift), C.byref(fills))
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_simulate_delivery_ext_host: error {rc}")
+    return dict(segments=segs, field_time_ns=times, dropped_protons=int(dropped.value), fixed_shift=int(shift.value),
+                fills=int(fills.value))
 
 
 class Context:
@@ -194,6 +235,19 @@ class Context:
         times = np.array([out.field_time_ns[i] for i in range(out.n_fields)], np.int64)
         return dict(segments=segs, field_time_ns=times, dropped_protons=int(out.dropped_protons),
                     fixed_shift=int(out.fixed_shift))
+
+    def simulate_delivery_ext(self, prm, total_histories, **ext_kw):
+        p = np.ascontiguousarray(prm, DELIV_DT)
+        x, keep = make_delivery_ext(**ext_kw)
+        out = PhaseLists(); fills = C.c_int64(0)
+        self._check(self.lib.pbs4d_simulate_delivery_ext(self.h, _np(p), C.byref(x), C.c_uint64(int(total_histories)),
+                                                         C.byref(out), C.byref(fills)))
+        segs = np.zeros(out.n_segments, SEG_DT)
+        if out.n_segments:
+            C.memmove(segs.ctypes.data, out.segments, segs.nbytes)
+        times = np.array([out.field_time_ns[i] for i in range(out.n_fields)], np.int64)
+        return dict(segments=segs, field_time_ns=times, dropped_protons=int(out.dropped_protons),
+                    fixed_shift=int(out.fixed_shift), fills=int(fills.value))
 
     # ---- a4-a7 ----
     def mc_dose_phase(self, phase, seed, per_protons=0.0, want_dose=True, want_rho=False):

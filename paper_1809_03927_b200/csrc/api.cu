@@ -283,16 +283,36 @@ int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags)
 // ------------------------------------------------------------------------------------------------------------------
 // a3: delivery simulation (host) and per-phase launch tables
 // ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm,
+                                           const pbs4d_delivery_ext* ext, uint64_t total_histories,
+                                           pbs4d_phase_lists* out, int64_t* n_fills);
+
 extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
                                        pbs4d_phase_lists* out)
+{
+    return pbs4d_simulate_delivery_ext(ctx, prm, nullptr, total_histories, out, nullptr);
+}
+
+// ext == NULL: the base simulator; else the extended model.  Both end in the same per-phase launch tables.
+extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm,
+                                           const pbs4d_delivery_ext* ext, uint64_t total_histories,
+                                           pbs4d_phase_lists* out, int64_t* n_fills)
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: null parameters");
     if (ctx->fields.empty()) return fail(ctx, PBS4D_ERR_ORDER, "simulate_delivery: call set_plan_spots first");
     if (total_histories > (uint64_t)1 << 62) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: too many histories");
     std::string err;
-    int rc = simulate_delivery_host(ctx->fields, ctx->spots, *prm, total_histories, ctx->segments, ctx->field_time,
+    int rc;
+    if (ext) {
+        int64_t fills = 0;
+        rc = simulate_delivery_ext_host(ctx->fields, ctx->spots, *prm, *ext, total_histories, ctx->segments,
+                                        ctx->field_time, ctx->dropped, fills, err);
+        if (n_fills) *n_fills = fills;
+    } else {
+        rc = simulate_delivery_host(ctx->fields, ctx->spots, *prm, total_histories, ctx->segments, ctx->field_time,
                                     ctx->dropped, err);
+    }
     if (rc != PBS4D_OK) return fail(ctx, rc, "simulate_delivery: " + err);
     ctx->fixed_shift = fixed_shift_for(ctx->segments, ctx->spots);
     ctx->deliv_phases = prm->n_phases;

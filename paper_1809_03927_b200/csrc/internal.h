@@ -19,6 +19,11 @@ int simulate_delivery_host(const std::vector<pbs4d_field>& fields, const std::ve
                            const pbs4d_delivery_params& prm, uint64_t total_histories,
                            std::vector<pbs4d_segment>& segments, std::vector<int64_t>& field_time_ns,
                            int64_t& dropped_protons, std::string& err);
+int simulate_delivery_ext_host(const std::vector<pbs4d_field>& fields, const std::vector<pbs4d_spot>& spots,
+                               const pbs4d_delivery_params& prm, const pbs4d_delivery_ext& ext,
+                               uint64_t total_histories, std::vector<pbs4d_segment>& segments,
+                               std::vector<int64_t>& field_time_ns, int64_t& dropped_protons, int64_t& n_fills,
+                               std::string& err);
 int32_t fixed_shift_for(const std::vector<pbs4d_segment>& segments, const std::vector<pbs4d_spot>& spots);
 
 // ---- device-side segment record (transport.cu): everything a history needs from its (field, spot) ----

@@ -21,7 +21,7 @@ def brute_force_ext(fields, spots, prm, cyc=None, discard=0, cap=0, flat=0, fixe
     counts, totals, fills = {}, [], 0
     for f in range(len(fields)):
         # explicit list of (start, end, phase) breathing bins, long enough for the plan
-        off = int(fields["start_phase"][f]) * (periods[0] // P)
+        off = (int(fields["start_phase"][f]) % P) * (periods[0] // P)        # phases count modulo N
         bins, b = [], 0
         for c in range(4000):
             tau = periods[min(c, len(periods) - 1)] // P
