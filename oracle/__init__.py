@@ -271,3 +271,19 @@ def simulate_delivery_ext(fields, spots, prm, total_histories, cycle_period_ns=N
     n2 = lib().orc_simulate_delivery_ext(*args, _p(segs), C.c_int64(n), _p(tt), C.byref(dropped), C.byref(fills))
     assert n2 == n
     return segs, tt, int(dropped.value), int(fills.value)
+
+
+DICOM_DVF_DT = np.dtype([("nx", "i4"), ("ny", "i4"), ("nz", "i4"), ("pad", "i4"), ("start", "f8", 3), ("delta", "f8", 3),
+                         ("row_cos", "f8", 3), ("col_cos", "f8", 3), ("pre", "f8", 16), ("post", "f8", 16)])
+
+
+def build_dvf(info, delta):
+    """Eq. 7-8: info = DICOM_DVF_DT record, delta [3, nz, ny, nx] fp32 -> (r_f, r_f - r_0) fp32"""
+    info = np.ascontiguousarray(info, DICOM_DVF_DT)
+    delta = np.ascontiguousarray(delta, np.float32)
+    rf = np.zeros_like(delta); disp = np.zeros_like(delta)
+    lib().orc_build_dvf.restype = C.c_int
+    rc = lib().orc_build_dvf(_p(info), _p(delta), _p(rf), _p(disp))
+    if rc != 0:
+        raise ValueError(f"orc_build_dvf: error {rc}")
+    return rf, disp

@@ -136,6 +136,18 @@ int orc_dim_pull(const orc_grid* R, int32_t nsx, int32_t nsy, int32_t nsz,
 int orc_dim_finalize(const orc_grid* R, const float* dose_ref, int32_t n_src, const double* pulled,
                      const orc_grid* dvf_grids, float* out);
 
+/* ---- DVF construction from DICOM minimal grid information, PAPER.md:251-259 (App. B, Eq. 7-8) ---- */
+typedef struct {
+    int32_t nx, ny, nz, pad;                 /* N_X (row direction), N_Y (column direction), N_Z (depth direction) */
+    double start[3];                         /* centre of the starting voxel, mm */
+    double delta[3];                         /* deformation-grid resolutions */
+    double row_cos[3], col_cos[3];           /* U, V; W = U x V */
+    double pre[16], post[16];                /* M_Pre, M_Post, row-major 4x4 */
+} orc_dicom_dvf;
+
+/* delta: translations [3][k][j][i] (fp32); rf / disp (either may be NULL): r_f and r_f - r_0, fp32 [3][k][j][i] */
+int orc_build_dvf(const orc_dicom_dvf* grid, const float* delta, float* rf, float* disp);
+
 #ifdef __cplusplus
 }
 #endif
