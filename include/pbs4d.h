@@ -215,6 +215,25 @@ int pbs4d_set_dvf_pull(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, con
 int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
                          const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats);
 
+/* ---- DVF construction (Sec. 2.D.1, App. B, Eq. 7-8) ----
+ * The minimal grid information a DICOM deformable spatial registration stores: starting voxel centre, resolutions,
+ * row/column direction cosines (depth = row x column), voxel counts, and the rigid pre-/post-deformation matrices
+ * (row-major 4x4; identity for registration between 4DCT phases). */
+typedef struct {
+    int32_t nx, ny, nz, pad;                 /* N_X along the row direction (fastest index), N_Y, N_Z */
+    double start[3], delta[3];               /* mm */
+    double row_cos[3], col_cos[3];
+    double pre[16], post[16];
+} pbs4d_dicom_dvf;
+
+/* One thread per deformation-grid voxel: r_0 by Eq. 8, r_f = M_Post (M_Pre r_0 + Delta) by Eq. 7, in double.
+ * delta_dev: stored translations [3][k][j][i] fp32.  rf_dev (optional): r_f; disp_dev (optional): r_f - r_0, both fp32
+ * [3][k][j][i].  grid_out (optional): when the direction cosines are the coordinate axes (row = +x, column = +y) the
+ * axis-aligned grid on which disp_dev can be passed to set_dvf / set_dvf_pull; otherwise PBS4D_ERR_ARG is returned
+ * if grid_out is requested (an oblique grid has no pbs4d_grid). */
+int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, const float* delta_dev, float* rf_dev, float* disp_dev,
+                    pbs4d_grid* grid_out);
+
 /* In-run roofline probes (BASELINE.json north_star: throughput is reported "as achieved fraction of the FP32-issue,
  * L2-atomic and HBM roofline measured by in-run microbenchmarks").  Each probe launches a small kernel of its own on
  * the context's stream, times it with CUDA events (best of 3-5 after a warm-up) and writes one number to *value:

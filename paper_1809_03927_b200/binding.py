@@ -23,13 +23,17 @@ DELIV_DT = np.dtype([("n_phases", "i4"), ("period_ns", "i8"), ("protons_per_weig
 SEG_DT = np.dtype([("field", "i4"), ("phase", "i4"), ("spot", "i4"), ("pad", "i4"), ("protons", "i8"),
                    ("first_history", "i8"), ("n_hist", "i8"), ("weight", "f8")])
 
+DICOM_DVF_DT = np.dtype([("nx", "i4"), ("ny", "i4"), ("nz", "i4"), ("pad", "i4"), ("start", "f8", 3), ("delta", "f8", 3),
+                         ("row_cos", "f8", 3), ("col_cos", "f8", 3), ("pre", "f8", 16), ("post", "f8", 16)])
+
 NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
 
 EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
            "pbs4d_mc_dose_phase", "pbs4d_mc_dose_phases", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
            "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe",
-           "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim", "pbs4d_simulate_delivery_ext", "pbs4d_simulate_delivery_ext_host"]
+           "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim", "pbs4d_simulate_delivery_ext", "pbs4d_simulate_delivery_ext_host",
+           "pbs4d_build_dvf"]
 
 
 class PhaseLists(C.Structure):
@@ -310,6 +314,18 @@ class Context:
         self._check(self.lib.pbs4d_get_accumulators(self.h, C.c_int32(src_phase), C.c_void_p(E.data_ptr()),
                                                     C.c_void_p(M.data_ptr())))
         return E, M
+
+    # ---- DVF construction (App. B) ----
+    def build_dvf(self, info, delta, want_grid=False):
+        """info: DICOM_DVF_DT record; delta: CUDA fp32 [3, nz, ny, nx] -> (r_f, r_f - r_0[, axis-aligned grid])"""
+        t = self.torch
+        r = np.ascontiguousarray(info, DICOM_DVF_DT)
+        self._dev(delta, t.float32)
+        rf = t.empty_like(delta); disp = t.empty_like(delta)
+        g = np.zeros(1, GRID_DT)
+        self._check(self.lib.pbs4d_build_dvf(self.h, _np(r), C.c_void_p(delta.data_ptr()), C.c_void_p(rf.data_ptr()),
+                                             C.c_void_p(disp.data_ptr()), _np(g) if want_grid else None))
+        return (rf, disp, g) if want_grid else (rf, disp)
 
     # ---- in-run roofline probes ----
     PROBES = {"fp32_issue": 0, "red_random": 1, "red_hot": 2, "hbm_copy": 3}

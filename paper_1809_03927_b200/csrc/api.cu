@@ -722,3 +722,31 @@ extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t n
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
     return PBS4D_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------------
+// DVF construction from DICOM minimal grid information
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, const float* delta_dev, float* rf_dev,
+                               float* disp_dev, pbs4d_grid* grid_out)
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!info || !delta_dev || (!rf_dev && !disp_dev) || info->nx < 1 || info->ny < 1 || info->nz < 1 ||
+        (double)info->nx * info->ny * info->nz >= 2.0e9 || !(info->delta[0] > 0.0) || !(info->delta[1] > 0.0) ||
+        !(info->delta[2] > 0.0))
+        return fail(ctx, PBS4D_ERR_ARG, "build_dvf: bad argument");
+    if (grid_out) {
+        const double* U = info->row_cos; const double* V = info->col_cos;
+        if (!(U[0] == 1.0 && U[1] == 0.0 && U[2] == 0.0 && V[0] == 0.0 && V[1] == 1.0 && V[2] == 0.0))
+            return fail(ctx, PBS4D_ERR_ARG, "build_dvf: grid_out needs direction cosines along +x, +y");
+        grid_out->nx = info->nx; grid_out->ny = info->ny; grid_out->nz = info->nz;
+        grid_out->hx = (float)info->delta[0]; grid_out->hy = (float)info->delta[1]; grid_out->hz = (float)info->delta[2];
+        grid_out->ox = (float)(info->start[0] - 0.5 * info->delta[0]);      // start = centre of the first voxel
+        grid_out->oy = (float)(info->start[1] - 0.5 * info->delta[1]);
+        grid_out->oz = (float)(info->start[2] - 0.5 * info->delta[2]);
+    }
+    CU(cudaSetDevice(ctx->device));
+    launch_dvf_build(*info, delta_dev, rf_dev, disp_dev, ctx->stream);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    return PBS4D_OK;
+}

@@ -86,6 +86,73 @@ __global__ void finalize_dose_kernel(long long nvox, const float* __restrict__ r
     }
 }
 
+
+// DVF construction (Sec. 2.D.1: "construct the DVFs ... one-thread-per-deformation-grid-voxel ... to
+// calculate r_f for all voxels"; App. B): Eq. 8 r_0 = start + i dX U + j dY V + k dZ W, W = U x V;
+// Eq. 7 r_f = M_Post (M_Pre [r_0; 1] + [Delta; 0]).  Double precision, one rounding per operation (this TU is built
+// with -fmad=false), outputs r_f and r_f - r_0 in fp32.  HBM-bound: 12 B read, 12-24 B written per grid voxel.
+struct DvfBuildParams {
+    int nx, ny, nz;
+    double start[3], delta[3], U[3], V[3], W[3], pre[16], post[16];
+    const float* __restrict__ dx; const float* __restrict__ dy; const float* __restrict__ dz;
+    float* rf; float* disp; size_t n;
+};
+
+__device__ __forceinline__ void mat4_apply(const double* M, const double v[4], double out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        double s = M[4 * r + 0] * v[0];
+        s = s + M[4 * r + 1] * v[1];
+        s = s + M[4 * r + 2] * v[2];
+        s = s + M[4 * r + 3] * v[3];
+        out[r] = s;
+    }
+}
+
+__global__ void __launch_bounds__(256) dvf_build_kernel(const __grid_constant__ DvfBuildParams P)
+{
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
+    const int j = blockIdx.x % P.ny, k = blockIdx.x / P.ny;          // rows on grid.x (up to 2^31 - 1)
+    if (i >= P.nx) return;
+    const size_t v = ((size_t)k * P.ny + j) * P.nx + i;
+    double r0[4], a[4], b[4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double s = P.U[c] * P.delta[0] * (double)i;
+        s = s + P.V[c] * P.delta[1] * (double)j;
+        s = s + P.W[c] * P.delta[2] * (double)k;
+        r0[c] = s + P.start[c];
+    }
+    r0[3] = 1.0;
+    mat4_apply(P.pre, r0, a);
+    a[0] = a[0] + (double)P.dx[v]; a[1] = a[1] + (double)P.dy[v]; a[2] = a[2] + (double)P.dz[v];
+    mat4_apply(P.post, a, b);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (P.rf)   P.rf[(size_t)c * P.n + v]   = (float)b[c];
+        if (P.disp) P.disp[(size_t)c * P.n + v] = (float)(b[c] - r0[c]);
+    }
+}
+
+}  // namespace
+
+void launch_dvf_build(const pbs4d_dicom_dvf& g, const float* delta_dev, float* rf_dev, float* disp_dev, cudaStream_t st)
+{
+    DvfBuildParams P;
+    P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.n = (size_t)g.nx * g.ny * g.nz;
+    for (int c = 0; c < 3; ++c) { P.start[c] = g.start[c]; P.delta[c] = g.delta[c]; P.U[c] = g.row_cos[c]; P.V[c] = g.col_cos[c]; }
+    P.W[0] = g.row_cos[1] * g.col_cos[2] - g.row_cos[2] * g.col_cos[1];
+    P.W[1] = g.row_cos[2] * g.col_cos[0] - g.row_cos[0] * g.col_cos[2];
+    P.W[2] = g.row_cos[0] * g.col_cos[1] - g.row_cos[1] * g.col_cos[0];
+    for (int e = 0; e < 16; ++e) { P.pre[e] = g.pre[e]; P.post[e] = g.post[e]; }
+    P.dx = delta_dev; P.dy = delta_dev + P.n; P.dz = delta_dev + 2 * P.n;
+    P.rf = rf_dev; P.disp = disp_dev;
+    dim3 grid((unsigned)(g.ny * g.nz), (g.nx + 255) / 256);
+    dvf_build_kernel<<<grid, 256, 0, st>>>(P);
+}
+
+namespace {
 }  // namespace
 
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,

@@ -66,6 +66,8 @@ void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_sr
                           const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev,
                           unsigned char* flags_dev /*[nx+ny+nz] scratch*/, float* out, cudaStream_t st);
 
+void launch_dvf_build(const pbs4d_dicom_dvf& g, const float* delta_dev, float* rf_dev, float* disp_dev, cudaStream_t st);
+
 // ---- dose-interpolation method (accumulate.cu) ----
 void launch_dim_init(const pbs4d_grid& ref, const float* dose_ref, double* acc, cudaStream_t st);
 void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs4d_grid& dvf_grid, const float* disp4,
