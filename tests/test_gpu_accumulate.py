@@ -136,3 +136,22 @@ def test_call_order_and_argument_errors(ctx):
     with pytest.raises(RuntimeError, match="-2"):
         fresh.mc_dose_phase(0, 1)                                    # no delivery yet
     fresh.close()
+
+
+def test_subdivision_convergence_as_in_the_paper(ctx):
+    # PAPER.md:167 (Sec. 3.B, Fig. 3): "EMTM with n = 1 ... differs", n = 2 already agrees with much finer
+    # subdivisions; the accumulation time grows as n^3.  Soft, qualitative check on config-4-like data:
+    # the n = 2 result is several times closer to the n = 8 result than the n = 1 result is, and n = 1 leaves holes
+    # (reference voxels that receive no mass) which n >= 2 fills.
+    c = synth.config4(n=64, n_phases=4, max_disp_mm=8.0)
+    out = {}
+    for n in (1, 2, 8):
+        o, st, EM = gpu_accumulate(ctx, c, (n, n, n))
+        out[n] = o.astype(np.float64)
+        holes = sum(int((EM[p][1] == 0).sum()) for p in EM)
+        out[(n, "holes")] = holes
+    inner = (slice(8, -8),) * 3                                   # away from the faces, where mass leaves the grid
+    d1 = np.abs(out[1] - out[8])[inner].mean(); d2 = np.abs(out[2] - out[8])[inner].mean()
+    assert d2 < 0.5 * d1, (d1, d2)
+    assert out[(1, "holes")] > 5 * max(out[(2, "holes")], 1) or out[(2, "holes")] < out[(1, "holes")]
+    assert out[(8, "holes")] <= out[(2, "holes")] <= out[(1, "holes")]
