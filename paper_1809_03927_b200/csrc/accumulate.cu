@@ -126,32 +126,41 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         const int rnx = P.ref.nx, rny = P.ref.ny;
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * nsy;
-        for (int c = 0; c < nsz; ++c) {
-            const AxisEntry mz = sz[c];
-            for (int b = 0; b < nsy; ++b) {
-                const AxisEntry my = syl[b];
-                const int r00 = (mz.i0 * dny + my.i0) * dnx;
-                const int sy1 = (my.flags & 1) * dnx, sz1 = (mz.flags & 1) * dny * dnx;
-                const float4* __restrict__ p00 = P.U + r00;              // the four x-rows of the cell
-                const float4* __restrict__ p01 = p00 + sy1;
-                const float4* __restrict__ p10 = p00 + sz1;
-                const float4* __restrict__ p11 = p10 + sy1;
-                const bool ok_zy = (mz.flags & my.flags & 2) != 0;
-                for (int a = 0; a < nsx; ++a) {
-                    const AxisEntry mx = sxl[a * kTileX];
-                    const bool ok = ok_zy && (mx.flags & 2);
-                    const int x0 = mx.i0;
-                    const float4 a000 = __ldg(p00 + x0), a001 = __ldg(p00 + x0 + dx1);
-                    const float4 a010 = __ldg(p01 + x0), a011 = __ldg(p01 + x0 + dx1);
-                    const float4 a100 = __ldg(p10 + x0), a101 = __ldg(p10 + x0 + dx1);
-                    const float4 a110 = __ldg(p11 + x0), a111 = __ldg(p11 + x0 + dx1);
-                    // per component: 4 lerps in x, 2 in y, 1 in z (A3), then q = p + u (A4)
-#define PBS4D_TRILERP(cmp) lerp_rn(lerp_rn(lerp_rn(a000.cmp, a001.cmp, mx.w), lerp_rn(a010.cmp, a011.cmp, mx.w), my.w), \
-                                   lerp_rn(lerp_rn(a100.cmp, a101.cmp, mx.w), lerp_rn(a110.cmp, a111.cmp, mx.w), my.w), mz.w)
-                    const float qx = __fadd_rn(mx.p, PBS4D_TRILERP(x));
-                    const float qy = __fadd_rn(my.p, PBS4D_TRILERP(y));
-                    const float qz = __fadd_rn(mz.p, PBS4D_TRILERP(z));
-#undef PBS4D_TRILERP
+        // Loop nest: y, x outside, z INSIDE.  The integer sums do not depend on the order in which subvoxels are
+        // visited, so the nest is arranged for reuse: all subvoxels of a (b, a) column that fall into the same DVF
+        // z-cell share the 8 corner vectors and the 6 x- and y-lerps per component (A3); only the z-lerp, q = p + u
+        // and the destination index are evaluated per subvoxel.  Each value is computed by exactly the operations
+        // of the contract, so the result stays bit-identical.
+        const int sz_stride = dny * dnx;
+        for (int b = 0; b < nsy; ++b) {
+            const AxisEntry my = syl[b];
+            const int sy1 = (my.flags & 1) * dnx;
+            for (int a = 0; a < nsx; ++a) {
+                const AxisEntry mx = sxl[a * kTileX];
+                const bool ok_xy = (mx.flags & my.flags & 2) != 0;
+                const float4* __restrict__ col = P.U + my.i0 * dnx + mx.i0;       // (y0, x0) of the column, z = 0
+                int cell_z = -1;
+                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f;
+                for (int c = 0; c < nsz; ++c) {
+                    const AxisEntry mz = sz[c];
+                    if (mz.i0 != cell_z) {                                        // new DVF z-cell: corners + x/y lerps
+                        cell_z = mz.i0;
+                        const float4* __restrict__ p00 = col + mz.i0 * sz_stride;
+                        const float4* __restrict__ p10 = p00 + (mz.flags & 1) * sz_stride;
+                        const float4 a000 = __ldg(p00), a001 = __ldg(p00 + dx1);
+                        const float4 a010 = __ldg(p00 + sy1), a011 = __ldg(p00 + sy1 + dx1);
+                        const float4 a100 = __ldg(p10), a101 = __ldg(p10 + dx1);
+                        const float4 a110 = __ldg(p10 + sy1), a111 = __ldg(p10 + sy1 + dx1);
+#define PBS4D_BILERP(A, B, C, D, cmp) lerp_rn(lerp_rn(A.cmp, B.cmp, mx.w), lerp_rn(C.cmp, D.cmp, mx.w), my.w)
+                        c0x = PBS4D_BILERP(a000, a001, a010, a011, x); c1x = PBS4D_BILERP(a100, a101, a110, a111, x);
+                        c0y = PBS4D_BILERP(a000, a001, a010, a011, y); c1y = PBS4D_BILERP(a100, a101, a110, a111, y);
+                        c0z = PBS4D_BILERP(a000, a001, a010, a011, z); c1z = PBS4D_BILERP(a100, a101, a110, a111, z);
+#undef PBS4D_BILERP
+                    }
+                    const bool ok = ok_xy && (mz.flags & 2);
+                    const float qx = __fadd_rn(mx.p, lerp_rn(c0x, c1x, mz.w));      // q = p + u (A4)
+                    const float qy = __fadd_rn(my.p, lerp_rn(c0y, c1y, mz.w));
+                    const float qz = __fadd_rn(mz.p, lerp_rn(c0z, c1z, mz.w));
                     const float fx = floor_quotient(__fsub_rn(qx, orx), hrx, ihx);
                     const float fy = floor_quotient(__fsub_rn(qy, ory), hry, ihy);
                     const float fz = floor_quotient(__fsub_rn(qz, orz), hrz, ihz);
