@@ -205,12 +205,14 @@ def main():
         n_hist = sum(st["histories"] for st in sts); n_steps = sum(st["steps"] for st in sts)
         n_red = sum(st["scoring_atomics"] for st in sts)
         out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
-        n_src = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])
+        n_dvf = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])      # fields re-laid out
+        g_ = ctx_shape(cfg)
+        n_src = int(ast["subvoxels"]) // (g_[0] * g_[1] * g_[2] * int(np.prod(cfg["subvox"])))   # phases really pushed
         # kernels launched: HU->density per phase, DVF interleave per source phase, transport + dose finalize per
         # phase run, push per source phase, coverage flags + accumulation finalize
         stats.update(histories=n_hist, mc_steps=n_steps, reds=n_red, transport_ms=t_ms, push_ms=ast["push_ms"],
                      finalize_ms=ast["finalize_ms"], phases=len(phases), n_src=n_src, subvoxels=ast["subvoxels"],
-                     launches=P + n_src + 2 * len(phases) + n_src + 2, checksum=float(out.sum()))
+                     launches=P + n_dvf + 2 * len(phases) + n_src + 2, checksum=float(out.sum()))
         return n_hist
 
     out_host = np.zeros(ctx_shape(cfg), np.float32)
