@@ -105,6 +105,13 @@ __device__ __forceinline__ void sincos_2pi(float u, float& s, float& c)
     s = -__sinf(a); c = -__cosf(a);
 }
 
+// the same angle 2 pi u - pi straight from the random word x, u = ((x >> 9) + 0.5) 2^-23: with f = 1 + (x >> 9) 2^-23
+// (built by bit operations) it is 2 pi f - 3 pi + pi 2^-23, one FMA
+__device__ __forceinline__ float angle_from_word(uint32_t x)
+{
+    return fmaf(__uint_as_float(0x3F800000u | (x >> 9)), kTwoPi, -9.42477758f);      // -3 pi + pi 2^-23
+}
+
 // table interval and fraction of an energy (integer operations on the bit pattern; see physics_tables.h)
 struct Lookup { int i; float f, inv_w; };
 __device__ __forceinline__ Lookup locate(float E)
@@ -126,7 +133,7 @@ struct Lane {
     uint32_t g_lo, g_hi, m;
     int vox;                                   // linear voxel index of the pending deposit (< 2^31 voxels)
     long long pend;                            // quanta deposited in vox and not yet flushed
-    float dens, inv_dens;
+    float dens, inv_dens;                      // dens holds 0.1 x density: t [g/cm2] = dens x s [mm]
     int seg;                                   // index of the history's segment in the launch table
 };
 
@@ -279,8 +286,7 @@ transport_kernel(const __grid_constant__ Params P)
                         L.wq = S.weight_scaled; L.seg = tag;
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.pend = 0;
-                        L.dens = __ldg(P.rho + L.vox);
-                        L.inv_dens = fast_rcp(L.dens);
+                        { const float rho = __ldg(P.rho + L.vox); L.dens = 0.1f * rho; L.inv_dens = fast_rcp(rho); }
                         alive = true;
                     }
                 }
@@ -327,7 +333,7 @@ transport_kernel(const __grid_constant__ Params P)
             const float s = crossing ? s_b : s_lim;
 
             // T7: midpoint-rule mean loss
-            const float t   = dens * s * 0.1f;                                // g/cm2
+            const float t   = dens * s;                                       // g/cm2 (dens = 0.1 rho)
             // E_m = E - S(E) t / 2 lies at most a few table intervals below E (an interval is 0.4-0.8 % of E, the
             // half-step loss <= ~0.7 % of E in water-like media): S, V, T at E_m are read off the SAME pair of nodes,
             // extrapolating linearly below the interval (error <= p(p-1)/2 (dE/E)^2 ~ 4e-5); only a half-step loss
@@ -348,7 +354,7 @@ transport_kernel(const __grid_constant__ Params P)
             float dE = dEm;
             if (do_strag) {
                 const float V2 = fmaf(fm, Bm.z - Am.z, Am.z);
-                const float a3 = fmaf(u01(r3), kTwoPi, -kPi);
+                const float a3 = angle_from_word(r3);
                 dE = fmaf(fast_sqrt(-V2 * t * fast_log2(u01(r2))), -__cosf(a3), dEm);
             }
             dE = fminf(fmaxf(dE, 0.0f), L.E);
@@ -356,7 +362,6 @@ transport_kernel(const __grid_constant__ Params P)
 
             // T9/T11: score into the voxel the step lay in (register accumulation, flushed on voxel change)
             L.pend += __float2ll_rn(dE * L.wq);
-            n_steps += 1;
 
             L.px = fmaf(s, L.dx, L.px); L.py = fmaf(s, L.dy, L.py); L.pz = fmaf(s, L.dz, L.pz);
 
@@ -378,7 +383,8 @@ transport_kernel(const __grid_constant__ Params P)
                 const float st  = th * fmaf(th2, fmaf(th2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
                 const float ct  = fmaf(th2, fmaf(th2, fmaf(th2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
                 float sp, cp;
-                sincos_2pi(u01(r1), sp, cp);
+                const float a1 = angle_from_word(r1);
+                sp = -__sinf(a1); cp = -__cosf(a1);
                 const float sw = copysignf(1.0f, L.dz);
                 const float aa = -fast_rcp(sw + L.dz);
                 const float bb = L.dx * L.dy * aa;
@@ -394,15 +400,16 @@ transport_kernel(const __grid_constant__ Params P)
 
             if (crossing || !alive) {
                 flush(P, L, q_dep, n_red);
+                if (!alive) n_steps += L.m;                                   // history absorbed: L.m = its step count
                 if (alive) {
                     if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
                         atomicAdd((unsigned long long*)&s_tally[4],                            // left the grid
                                   (unsigned long long)__double2ll_rn((double)L.E * P.segs[L.seg].weight_scaled_d));
                         alive = false;
+                        n_steps += L.m;
                     } else {
                         L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
-                        L.dens = __ldg(P.rho + L.vox);
-                        L.inv_dens = fast_rcp(L.dens);
+                        { const float rho = __ldg(P.rho + L.vox); L.dens = 0.1f * rho; L.inv_dens = fast_rcp(rho); }
                     }
                 }
             }
