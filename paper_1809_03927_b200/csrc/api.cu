@@ -32,6 +32,17 @@ struct DevBuf {                          // RAII device allocation
     template <class T> T* as() const { return static_cast<T*>(p); }
 };
 
+struct EventTrio {                       // RAII: three timing events
+    cudaEvent_t e[3] = { nullptr, nullptr, nullptr };
+    EventTrio() = default;
+    EventTrio(const EventTrio&) = delete; EventTrio& operator=(const EventTrio&) = delete;
+    cudaError_t create() {
+        for (auto& x : e) { cudaError_t rc = cudaEventCreate(&x); if (rc != cudaSuccess) return rc; }
+        return cudaSuccess;
+    }
+    ~EventTrio() { for (auto x : e) if (x) cudaEventDestroy(x); }
+};
+
 struct PhaseLaunch {                     // per-phase segment table for the transport kernel
     std::vector<DevSegment> segs;
     std::vector<long long> seg_begin;    // segs[i].local_begin, contiguous for the kernel's binary search
@@ -507,8 +518,9 @@ extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int3
     const size_t nvox = ctx->nvox();
     CU(ctx->acc_counters.ensure(sizeof(AccCounters)));
     CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
-    cudaEvent_t e0, e1, e2;
-    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1)); CU(cudaEventCreate(&e2));
+    EventTrio ev;                                        // destroyed on every return path
+    CU(ev.create());
+    cudaEvent_t e0 = ev.e[0], e1 = ev.e[1], e2 = ev.e[2];
     std::fill(ctx->have_acc.begin(), ctx->have_acc.end(), false);
     for (int p : src) {
         CU(ctx->accE[p]->ensure(nvox * sizeof(long long)));
@@ -542,7 +554,6 @@ extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int3
         cudaEventElapsedTime(&stats->push_ms, e0, e1);
         cudaEventElapsedTime(&stats->finalize_ms, e1, e2);
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
     return PBS4D_OK;
 }
 
@@ -694,8 +705,9 @@ extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t n
     CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
     CU(ctx->dim_acc.ensure(nvox * sizeof(double)));
     CU(ctx->cover_flags.ensure((size_t)ctx->dose_grid.nx + ctx->dose_grid.ny + ctx->dose_grid.nz));
-    cudaEvent_t e0, e1, e2;
-    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1)); CU(cudaEventCreate(&e2));
+    EventTrio ev;                                        // destroyed on every return path
+    CU(ev.create());
+    cudaEvent_t e0 = ev.e[0], e1 = ev.e[1], e2 = ev.e[2];
     launch_dim_init(ctx->dose_grid, dose_of(ref_phase), ctx->dim_acc.as<double>(), ctx->stream);
     CU(cudaEventRecord(e0, ctx->stream));
     std::vector<pbs4d_grid> dg;
@@ -719,7 +731,6 @@ extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t n
         cudaEventElapsedTime(&stats->push_ms, e0, e1);
         cudaEventElapsedTime(&stats->finalize_ms, e1, e2);
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
     return PBS4D_OK;
 }
 
