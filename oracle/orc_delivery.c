@@ -73,7 +73,7 @@ int64_t orc_simulate_delivery(int32_t n_fields, const orc_field* fields, int64_t
 
     for (int32_t f = 0; f < n_fields; ++f) {
         int64_t t = 0;                                                /* D2: each field starts at t = 0 */
-        const int32_t sp0 = fields[f].start_phase;
+        int32_t sp0 = fields[f].start_phase % P; if (sp0 < 0) sp0 += P;   /* phases are counted modulo N (B2), as in _ext */
         int first_layer = 1;
         int64_t s = 0;
         while (s < n_spots) {

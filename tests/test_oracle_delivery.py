@@ -138,6 +138,13 @@ def test_start_phase_rotates_the_lists():
     da = {((int(s["phase"]) + 4) % 6, int(s["spot"])): int(s["protons"]) for s in a}
     db = {(int(s["phase"]), int(s["spot"])): int(s["protons"]) for s in b}
     assert da == db
+    # phases are counted modulo N (reading B2): start phases -2 and 10 are start phase 4 of 6, in both oracle entries
+    for sp in (-2, 10):
+        f3 = fields.copy(); f3["start_phase"] = sp
+        c, _, _ = orc.simulate_delivery(f3, spots, prm, 0)
+        assert c.tobytes() == b.tobytes()
+        cx, _, _, _ = orc.simulate_delivery_ext(f3, spots, prm, 0)
+        assert cx.tobytes() == b.tobytes()
 
 
 def test_history_allocation_d7():
