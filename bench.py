@@ -21,12 +21,28 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# algorithmic work of one condensed-history step, in fp32/int32 lane-operations
-OPS_PER_STEP = 262
-# dram__bytes_read.sum + dram__bytes_write.sum of one transport_kernel launch (ncu --set full, profiles/)
+# hand-count MODEL of the lane-operations of one condensed-history step; used only when the ncu
+# summary under profiles/ is missing -- the reported figure is the measured one (profile_metrics)
+OPS_PER_STEP_MODEL = 262
 # histories of the bounded oracle sample (10-30 s of host work on 16 cores); the reference arm uses half per step
 ORACLE_SAMPLE = {"config5": 200_000, "config3": 400_000, "config2": 200_000}
-TRANSPORT_DRAM_BYTES_PER_LAUNCH = {"config3": 7.6e6, "config5": 74.8e6}
+# per-kernel numbers taken from the committed ncu captures (kernel, workload, metric, value); written by hand from the
+# reports named in profiles/r2_summary.md
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernel_metrics.csv")
+
+
+def profile_metrics():
+    """{(kernel, workload, metric): value} from profiles/r2_kernel_metrics.csv; {} if the file is absent"""
+    out = {}
+    try:
+        with open(PROFILE_CSV) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 4 and not line.startswith("#") and c[0] != "kernel":
+                    out[(c[0], c[1], c[2])] = float(c[3])
+    except OSError:
+        pass
+    return out
 
 
 def parse():
@@ -120,9 +136,43 @@ def oracle_sample(cfg, budget_hist):
                              f"(delivery + HU->density + transport; {wall:.1f} s wall, transport {t_tr:.1f} s)")
 
 
+def source_owners(src_phases, world):
+    """accumulation shards by source phase: the i-th source phase (ascending) is pushed by rank i % world"""
+    return {p: i % world for i, p in enumerate(sorted(src_phases))}
+
+
+def owner_mask(owners, rank):
+    m = 0
+    for p, r in owners.items():
+        if r == rank:
+            m |= 1 << p
+    return m
+
+
+def sum_energy_grids(grids, world):
+    """integer all-reduce (SUM) of the int64 energy grids of the phases, in place: exact and order-independent, so
+    every rank ends up with the grid of the unsharded run bit for bit"""
+    if world <= 1:
+        return
+    import torch.distributed as dist
+    for q in grids:
+        assert q.dtype.is_floating_point is False and q.element_size() == 8
+        dist.all_reduce(q, op=dist.ReduceOp.SUM)
+
+
+def share_accumulators(pairs, owners, world):
+    """pairs: {source phase: (E, M)} int64 sums; broadcast each from the rank that pushed it"""
+    if world <= 1:
+        return
+    import torch.distributed as dist
+    for p in sorted(pairs):
+        for t in pairs[p]:
+            dist.broadcast(t, src=owners[p])
+
+
 def reduce_over_ranks(ms, e2e_s, hist, hist_e2e, world, device):
-    """Replicas: every rank ran an independent plan.  Times -> MAX over ranks, histories -> SUM over ranks
-    (whole-job throughput = all histories / slowest rank's time).  The only collectives of the whole program."""
+    """Times -> MAX over ranks, histories -> SUM over ranks (whole-job throughput = all histories / slowest rank's
+    time)."""
     if world <= 1:
         return ms, e2e_s, hist, hist_e2e
     import torch
@@ -180,20 +230,25 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- inputs: every rank runs an independent plan (replicas / weak scaling) ----
-    cfg = make_workload(args.workload, rank, args.histories)
+    # ---- inputs.  N = 1: the plan of the workload.  N > 1: STRONG scaling -- every rank holds the same plan and
+    # transports its slice of every phase's history range; the int64 energy grids are summed over the ranks with one
+    # integer all-reduce per phase (NCCL), the accumulation is sharded by source phase and its int64 sums are
+    # broadcast from their owners ----
+    cfg = make_workload(args.workload, 0, args.histories)
     P = cfg["hu"].shape[0]
     ctx = binding.Context(local_rank)
     hu_dev = torch.from_numpy(cfg["hu"]).cuda()
     dvf_dev = [None if d is None else torch.from_numpy(d).cuda() for d in cfg["dvf"]]
     hu_host = [cfg["hu"][p] for p in range(P)]
-    h2d = cfg["hu"].nbytes + sum(d.nbytes for d in cfg["dvf"] if d is not None) + cfg["spots"].nbytes + cfg["fields"].nbytes
     for a in hu_host + [d for d in cfg["dvf"] if d is not None]:
         torch.cuda.cudart().cudaHostRegister(a.ctypes.data, a.nbytes, 0)          # pinned host inputs
+    nvox = int(np.prod(ctx_shape(cfg)))
+    n_sub = int(np.prod(cfg["subvox"]))
 
     stats = {}
 
     def step_device():
+        """one pass of the whole path, inputs resident in HBM"""
         ctx.set_ct_phases(cfg["ct_grid"], [hu_dev[p] for p in range(P)], cfg["dose_grid"])
         for p in range(P):
             if dvf_dev[p] is not None:
@@ -201,30 +256,61 @@ def main():
         ctx.set_plan_spots(cfg["fields"], cfg["spots"])
         deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
         phases = sorted(set(int(x) for x in deliv["segments"]["phase"]) | {cfg["ref_phase"]})
+        ctx.set_shard(rank, world)
         sts, t_ms = ctx.mc_dose_phases(phases, cfg["seed"])          # all phases, concurrent launches; t_ms = fork..join
         n_hist = sum(st["histories"] for st in sts); n_steps = sum(st["steps"] for st in sts)
         n_red = sum(st["scoring_atomics"] for st in sts)
-        out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
         n_dvf = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])      # fields re-laid out
-        g_ = ctx_shape(cfg)
-        n_src = int(ast["subvoxels"]) // (g_[0] * g_[1] * g_[2] * int(np.prod(cfg["subvox"])))   # phases really pushed
+        src = [p for p in phases if p != cfg["ref_phase"] and dvf_dev[p] is not None]
+        extra = 0
+        if world == 1:
+            out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
+            n_src = int(ast["subvoxels"]) // (nvox * n_sub)                                       # phases really pushed
+        else:
+            sum_energy_grids([ctx.phase_energy_view(p) for p in phases], world)                   # the exchange step
+            for p in phases:
+                ctx.finalize_phase_dose(p)
+            owners = source_owners(src, world)
+            ast = ctx.accumulate_push(cfg["ref_phase"], cfg["subvox"], owner_mask(owners, rank))
+            share_accumulators({p: ctx.accumulator_views(p) for p in src}, owners, world)
+            out, fst = ctx.accumulate_finalize(cfg["ref_phase"])
+            ast["finalize_ms"] = fst["finalize_ms"]
+            n_src = int(ast["subvoxels"]) // (nvox * n_sub)
+            extra = len(phases)                                                                    # second a7 launches
         # kernels launched: HU->density per phase, DVF interleave per source phase, transport + dose finalize per
-        # phase run, push per source phase, coverage flags + accumulation finalize
+        # phase run, push per source phase pushed here, coverage flags + accumulation finalize
+        n_tr = sum(1 for st in sts if st["histories"] > 0)
         stats.update(histories=n_hist, mc_steps=n_steps, reds=n_red, transport_ms=t_ms, push_ms=ast["push_ms"],
                      finalize_ms=ast["finalize_ms"], phases=len(phases), n_src=n_src, subvoxels=ast["subvoxels"],
-                     launches=P + n_dvf + 2 * len(phases) + n_src + 2, checksum=float(out.sum()))
-        return n_hist
+                     launches=P + n_dvf + n_tr + len(phases) + extra + n_src + 2, checksum=float(out.sum()),
+                     active=phases, src=src)
+        return n_hist, out
 
     out_host = np.zeros(ctx_shape(cfg), np.float32)
     torch.cuda.cudart().cudaHostRegister(out_host.ctypes.data, out_host.nbytes, 0)
+    out_pinned = torch.from_numpy(out_host)
 
     def step_e2e():
-        run, secs = ctx.run_plan_host(cfg["ct_grid"], hu_host, cfg["dose_grid"], cfg["dvf_grid"],
-                                      cfg["dvf"] if cfg["dvf_grid"] is not None else None, cfg["ref_phase"],
-                                      cfg["fields"], cfg["spots"], cfg["deliv"], cfg["histories"], cfg["seed"],
-                                      cfg["subvox"], out_host)
-        stats["e2e_seconds"] = secs
-        return run
+        """the same pass from HOST buffers, copies inside.  N = 1: the C-ABI entry pbs4d_run_plan_host.  N > 1: every
+        rank uploads the plan's inputs from pinned host memory, runs its shard, rank 0 reads the 4D dose back."""
+        if world == 1:
+            run, secs, h2d = ctx.run_plan_host(cfg["ct_grid"], hu_host, cfg["dose_grid"], cfg["dvf_grid"],
+                                               cfg["dvf"] if cfg["dvf_grid"] is not None else None, cfg["ref_phase"],
+                                               cfg["fields"], cfg["spots"], cfg["deliv"], cfg["histories"],
+                                               cfg["seed"], cfg["subvox"], out_host)
+            stats.update(e2e_seconds=secs, h2d=h2d)
+            return run
+        h2d = cfg["spots"].nbytes + cfg["fields"].nbytes
+        for p in range(P):
+            hu_dev[p].copy_(torch.from_numpy(hu_host[p]), non_blocking=True); h2d += hu_host[p].nbytes
+            if dvf_dev[p] is not None:
+                dvf_dev[p].copy_(torch.from_numpy(cfg["dvf"][p]), non_blocking=True); h2d += cfg["dvf"][p].nbytes
+        n, out = step_device()
+        if rank == 0:
+            out_pinned.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+        stats.update(h2d=h2d)
+        return n
 
     # ---- in-run roofline probes (small kernels of the library itself, before the timed region) ----
     probes = {k: ctx.roofline_probe(k) for k in ("fp32_issue", "red_random", "red_hot", "hbm_copy")}
@@ -236,15 +322,16 @@ def main():
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    hist = 0; tr_ms = 0.0; mc_steps = 0; reds = 0
+    hist = 0; tr_ms = 0.0; mc_steps = 0; reds = 0; launches = 0
     for _ in range(args.steps):
-        hist += step_device(); tr_ms += stats["transport_ms"]; mc_steps += stats["mc_steps"]; reds += stats["reds"]
+        hist += step_device()[0]; tr_ms += stats["transport_ms"]; mc_steps += stats["mc_steps"]; reds += stats["reds"]
+        launches += stats["launches"]
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.summary()
 
-    # ---- end-to-end timing (host buffers through the C-ABI) ----
+    # ---- end-to-end timing (host buffers) ----
     step_e2e()
     barrier()
     t0 = time.perf_counter()
@@ -255,57 +342,87 @@ def main():
     e2e_s = time.perf_counter() - t0
 
     ms, e2e_s, hist, hist_e2e = reduce_over_ranks(ms, e2e_s, hist, hist_e2e, world, torch.device("cuda", local_rank))
+    if world > 1:                                         # per-rank launch counts and transport steps -> whole job
+        tot = torch.tensor([float(launches), float(mc_steps), float(reds)], dtype=torch.float64, device="cuda")
+        tmax = torch.tensor([tr_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        launches, mc_steps, reds, tr_ms = int(tot[0]), float(tot[1]), float(tot[2]), float(tmax[0])
     if rank != 0:
+        ctx.close()
+        dist.destroy_process_group()
         return
 
     peaks, peak_kind = measured_peaks()
+    prof = profile_metrics()
+    wl = args.workload
     sm_mhz = clocks["sm_mhz"] or peaks.get("sm_max_mhz", 1965.0)
     steps_per_s = mc_steps / (tr_ms * 1e-3)
-    achieved = steps_per_s * OPS_PER_STEP / 1e12
     props = torch.cuda.get_device_properties(local_rank)
-    nvox = int(np.prod(ctx_shape(cfg)))
+    peak = world * props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
+    # lane-instructions per condensed-history step: executed thread instructions of the transport kernel / steps, from
+    # the committed ncu capture of the kernel (profiles/); the hand-count model only when that file is missing
+    ops_step = prof.get(("transport_kernel", wl, "thread_inst_per_step")) or \
+        prof.get(("transport_kernel", "config5", "thread_inst_per_step"))
+    ops_kind = "ncu smsp__thread_inst_executed / steps (profiles/r2_kernel_metrics.csv)"
+    if not ops_step:
+        ops_step, ops_kind = OPS_PER_STEP_MODEL, "hand-count model (no ncu capture found)"
+    achieved = steps_per_s * ops_step / 1e12
     acc_bytes = stats["n_src"] * nvox * (20 + 16)
-    fin_bytes = nvox * (16 * stats["n_src"] + 8)
-    peak = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
+    fin_bytes = nvox * (16 * len(stats["src"]) + 8)
+    push_s = stats["push_ms"] * 1e-3
+    sub_key = "x".join(str(v) for v in cfg["subvox"])
+    push_ops = prof.get(("emtm_push_kernel", f"{wl}_{sub_key}", "thread_inst_per_subvoxel"))
+    push_peak = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
     line = {
         "metric": "proton histories/s", "value": hist / (ms * 1e-3), "unit": "histories/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": args.workload, "histories_per_step": stats["histories"], "phases_run": stats["phases"],
-                   "source_phases": stats["n_src"], "subvoxels": list(cfg["subvox"]),
+        "scaling": "strong" if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl, "histories_per_step": int(hist / args.steps), "phases_run": stats["phases"],
+                   "source_phases": len(stats["src"]), "subvoxels": list(cfg["subvox"]),
                    "l2": "per-step working set (CT int16 + DVFs + int64 grids) exceeds the 126 MB L2"
-                         if args.workload != "config2" else "inputs smaller than L2 (parity config)",
-                   "parallelism": "replicas" if world > 1 else "single"},
-        "e2e": {"value": hist_e2e / e2e_s, "unit": "histories/s", "h2d_bytes_per_step": int(h2d),
+                         if wl != "config2" else "inputs smaller than L2 (parity config)",
+                   "parallelism": (f"one plan sharded over {world} ranks: history slices + int64 all-reduce of the "
+                                   "energy grids, accumulation by source phase") if world > 1 else "single"},
+        "e2e": {"value": hist_e2e / e2e_s, "unit": "histories/s", "h2d_bytes_per_step": int(stats["h2d"]),
                 "d2h_bytes_per_step": int(out_host.nbytes), "seconds_per_plan": e2e_s / args.steps,
-                "split_s": stats.get("e2e_seconds")},
+                "split_s": stats.get("e2e_seconds"),
+                "note": "h2d bytes are those actually copied: CT and DVF of the phases that receive beam"},
         "seconds_per_plan_device": ms * 1e-3 / args.steps,
-        "gpu_launches": stats["launches"] * args.steps,
+        "gpu_launches": launches,
         "kernel_ms_per_step": {"transport": tr_ms / args.steps, "push": stats["push_ms"], "acc_finalize": stats["finalize_ms"]},
-        "transport_histories_per_s": hist / world / (tr_ms * 1e-3) if world == 1 else None,
+        "transport_histories_per_s": hist / (tr_ms * 1e-3),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
-                     "traffic": TRANSPORT_DRAM_BYTES_PER_LAUNCH.get(args.workload), "kernel": "transport_kernel",
-                     "how": f"{OPS_PER_STEP} algorithmic lane-ops/step x {steps_per_s:.3e} steps/s over the CUDA-event time of the "
+                     "traffic": prof.get(("transport_kernel", wl, "dram_bytes_per_launch")), "kernel": "transport_kernel",
+                     "lane_ops_per_step": ops_step, "lane_ops_source": ops_kind,
+                     "how": f"{ops_step:.1f} executed lane-instructions per step x {steps_per_s:.3e} steps/s over the CUDA-event time of the "
                             f"transport launches of a pass (fork to join of the per-phase kernels, which overlap at their tails); peak = SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz, {peak_kind} peaks file); "
                             "traffic = dram bytes read+written per launch from the ncu --set full capture under profiles/",
                      "measured_fp32_issue": probes["fp32_issue"] / 1e12,
-                     "frac_of_measured_fp32_issue": achieved / (probes["fp32_issue"] / 1e12),
+                     "frac_of_measured_fp32_issue": achieved / (world * probes["fp32_issue"] / 1e12),
                      "scoring_atomics_per_s": reds / (tr_ms * 1e-3), "measured_red_random_per_s": probes["red_random"],
                      "measured_red_hot_per_s": probes["red_hot"],
-                     "atomic_frac": reds / (tr_ms * 1e-3) / probes["red_random"]},
-        "roofline_accumulate": {"bound": "hbm" if max(cfg["subvox"]) <= 2 else "alu", "kernel": "emtm_push_kernel",
-                                "achieved": acc_bytes / (stats["push_ms"] * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
-                                "unit": "GB/s", "frac": acc_bytes / (stats["push_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                     "atomic_frac": reds / (tr_ms * 1e-3) / (world * probes["red_random"])},
+        # the push kernel against BOTH rooflines: algorithmic HBM bytes and executed lane-instructions
+        "roofline_accumulate": {"kernel": "emtm_push_kernel", "subvoxels": list(cfg["subvox"]),
+                                "hbm": {"bound": "hbm", "achieved": acc_bytes / push_s / 1e9, "peak": peaks["hbm_gbs"],
+                                        "unit": "GB/s", "frac": acc_bytes / push_s / 1e9 / peaks["hbm_gbs"],
+                                        "traffic": prof.get(("emtm_push_kernel", f"{wl}_{sub_key}", "dram_bytes_per_launch"))},
+                                "issue": None if not push_ops else
+                                {"bound": "alu", "achieved": stats["subvoxels"] / push_s * push_ops / 1e12, "peak": push_peak,
+                                 "unit": "Tlane-op/s", "frac": stats["subvoxels"] / push_s * push_ops / 1e12 / push_peak,
+                                 "lane_ops_per_subvoxel": push_ops},
+                                "binding": "alu" if push_ops else "unknown (no ncu capture for this subdivision)",
                                 "measured_hbm_copy": probes["hbm_copy"] / 1e9,
-                                "subvoxels_per_s": stats["subvoxels"] / (stats["push_ms"] * 1e-3),
+                                "subvoxels_per_s": stats["subvoxels"] / push_s,
                                 "finalize_GBps": fin_bytes / (stats["finalize_ms"] * 1e-3) / 1e9,
-                                "how": "algorithmic bytes = 20 B per source voxel (dose, density, 3 DVF components) + 16 B "
+                                "how": "hbm: algorithmic bytes = 20 B per source voxel (dose, density, 3 DVF components) + 16 B "
                                        "read-modify-write per reference voxel, per source phase, over the push kernels' "
-                                       "CUDA-event time; finalize = (16 n_src + 8) B per voxel"},
+                                       "CUDA-event time; issue: executed lane-instructions per subvoxel from the ncu capture "
+                                       "under profiles/ x subvoxels/s; finalize = (16 n_src + 8) B per voxel"},
     }
     if not args.no_cpu_baseline and world == 1:
-        r, cores, text = oracle_sample(cfg, ORACLE_SAMPLE[args.workload])
+        r, cores, text = oracle_sample(cfg, ORACLE_SAMPLE[wl])
         line["cpu_baseline"] = {"value": r, "unit": "histories/s", "cores": cores, "kind": "oracle", "sample": text}
     print(json.dumps(line), flush=True)
     ctx.close()

@@ -31,6 +31,7 @@ extern "C" {
 
 typedef struct pbs4d_ctx pbs4d_ctx;      /* opaque; owns all internal host/device memory */
 
+/* at most 4e6 voxels per axis and 2e9 in total */
 typedef struct { int32_t nx, ny, nz; float hx, hy, hz, ox, oy, oz; } pbs4d_grid;
 
 /* A treatment field: parallel beam along dir; (eu, ev) span the beam's-eye-view plane through ref.
@@ -120,7 +121,9 @@ const char* pbs4d_last_error(const pbs4d_ctx* ctx);
 int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_dev,
                         const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts);
 
-/* Alternative to set_ct_phases: densities given directly on the dose grid (rho_dev[p] -> fp32 [z][y][x]); copied. */
+/* Alternative to set_ct_phases: densities given directly on the dose grid (rho_dev[p] -> fp32 [z][y][x]); copied.
+ * Every density must be finite and within [1e-6, 100] g/cm3 (checked on the device; PBS4D_ERR_ARG otherwise): a zero
+ * density has no dose (0/0), an infinite one a zero step limit. */
 int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* dose_grid,
                              const float* const* rho_dev);
 
@@ -160,6 +163,55 @@ int pbs4d_simulate_delivery_ext_host(int32_t n_fields, const pbs4d_field* fields
                                      int64_t* field_time_ns, int64_t* dropped_protons, int32_t* fixed_shift,
                                      int64_t* n_fills);
 
+/* ---- uncertainty trials ----
+ * "The effect of these uncertainties was considered by running 25 trials of the 4DDC where, for each trial, the
+ * initial-breathing phase, breathing period, and synchrotron delivery parameters were simultaneously varied according
+ * to their statistical distributions ...: starting phase ~ U(CT_0, CT_90), synchrotron parameters ~ N(mu, sigma), and
+ * breathing period ~ U(3,7) s" (discrete uniforms, inclusive); "t_ph ~ N(mu, sigma)/N" per breathing cycle
+ * (PAPER.md:55).  Ref. 45's central values and uncertainties are not available: they are inputs.  Every draw is one
+ * Philox4x32-10 block addressed by (what, which, trial) under `seed`, so a trial can be sampled on its own. */
+typedef struct {
+    uint64_t seed;
+    int32_t  n_trials;              /* T (25 in the paper)                                                    */
+    int32_t  n_cycles;              /* breathing cycles sampled per trial (the last one repeats); 0: regular   */
+    int64_t  period_lo_ns, period_hi_ns, period_step_ns;   /* mean period ~ U{lo, lo + step, ... <= hi}; lo = 0: the
+                                                              plan's period_ns, not sampled                     */
+    int64_t  period_sigma_ns;       /* per-cycle period ~ N(mean period, sigma), floored at a quarter of the mean */
+    int64_t  discard_sigma_ns, flat_top_sigma_ns, spot_switch_sigma_ns, layer_switch_sigma_ns;
+    int64_t  spill_protons_sigma, protons_per_s_sigma;     /* 1-sigma uncertainties of the parameters; 0 = fixed */
+} pbs4d_trial_spec;
+
+/* Device-free: sample trial `trial` (0 <= trial < n_trials) around the central values prm / ext.  The caller's arrays
+ * start_phase[n_fields], cycle_period_ns[spec->n_cycles], layer_switch_ns[ext->n_layer_switch] receive the draws;
+ * *prm_out / *ext_out are copies of prm / ext with the sampled values whose pointers refer to those arrays.  Sampled
+ * values are clamped so that every trial can be delivered (discard < shortest phase, flat-top > longest period). */
+int pbs4d_sample_delivery_trial(const pbs4d_trial_spec* spec, int32_t trial, int32_t n_fields,
+                                const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
+                                int32_t* start_phase, int64_t* cycle_period_ns, int64_t* layer_switch_ns,
+                                pbs4d_delivery_params* prm_out, pbs4d_delivery_ext* ext_out);
+
+/* a3 for one trial: sample it, start every field in its sampled phase and run the extended delivery simulation. */
+int pbs4d_simulate_delivery_trial(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, int32_t trial,
+                                  const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
+                                  uint64_t total_histories, pbs4d_phase_lists* out, int64_t* n_fills);
+
+typedef struct {
+    uint64_t histories;             /* histories transported in this trial                                    */
+    int64_t  delivery_ns;           /* end of delivery of the slowest field                                   */
+    int64_t  fills;                 /* synchrotron fills of all fields                                        */
+    int32_t  phases_run, pad;       /* phases that received beam                                              */
+    float    transport_ms, accumulate_ms;   /* device times                                                   */
+} pbs4d_trial_result;
+
+/* The trial loop: for trial = first .. first + count - 1: simulate_delivery_trial, mc_dose_phases (Philox key
+ * seed + trial) on every phase that receives beam plus ref_phase, accumulate_subvoxel onto ref_phase; the 4D dose of
+ * trial t goes to dose4d_dev[t - first] (fp32 [z][y][x], caller's buffers).  Densities, DVFs and the plan must have
+ * been set; the context is re-used across trials (no allocation after the first).  results (optional) -> [count]. */
+int pbs4d_run_trials(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, int32_t first, int32_t count,
+                     const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext, uint64_t total_histories,
+                     uint64_t seed, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                     float* const* dose4d_dev, pbs4d_trial_result* results);
+
 /* a4-a7: Monte Carlo transport of all segments of `phase` on that phase's density grid.
  * dose_dev (optional) receives fp32 Gy [z][y][x] on the dose grid for the delivered protons (divided by
  * per_protons if > 0, e.g. "Gy per proton"); rho_dev (optional) receives the density grid (dose and
@@ -188,16 +240,57 @@ int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, in
 /* Integer energy/mass sums of the last accumulate_subvoxel for one source phase (int64 [z][y][x] each). */
 int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev);
 
-/* Whole path with HOST buffers (copies inside): set_ct_phases + set_dvf + set_plan_spots + simulate_delivery +
- * mc_dose_phase for every phase with protons + accumulate_subvoxel.  hu_host[p], disp_host[p] (NULL = no DVF for p),
- * dose4d_host out.  seconds (optional, [4]): h2d, delivery, transport, accumulate+d2h wall times. */
+/* ---- multi-GPU sharding ("N_g simulations per field", "the MC was distributed amongst eight
+ * GPUs").  One process per GPU, each with its own context holding the whole plan.  Histories are
+ * independent units (one Philox counter each), so rank r of w transports the contiguous slice
+ * [floor(n r / w), floor(n (r+1) / w)) of every phase's n local histories; the int64 energy grids of the ranks then
+ * add up to the unsharded grid BIT FOR BIT.  The caller sums them in place (an integer all-reduce over
+ * pbs4d_phase_energy_ptr, e.g. NCCL through torch.distributed) and re-derives the dose with
+ * pbs4d_finalize_phase_dose.  Accumulation shards by source phase: pbs4d_accumulate_push with the rank's src_mask,
+ * exchange of the int64 sums (pbs4d_accumulator_ptrs: broadcast from the owner or all-reduce, the other ranks hold
+ * zeros), then pbs4d_accumulate_finalize on every rank. */
+
+/* Device-free partition arithmetic: *begin, *count of rank's slice of n_hist histories (every history exactly once
+ * over the ranks; empty slices when world > n_hist). */
+int pbs4d_shard_window(int64_t n_hist, int32_t rank, int32_t world, int64_t* begin, int64_t* count);
+
+/* Subsequent mc_dose_phase(s) transport only this rank's slice of every phase (default rank 0 of 1 = everything).
+ * Stats then count the slice; doses kept by the context are partial until the grids have been summed. */
+int pbs4d_set_shard(pbs4d_ctx* ctx, int32_t rank, int32_t world);
+
+/* Device pointer to the context's own int64 energy grid [z][y][x] of `phase` (valid until the next set_ct_phases /
+ * set_density_phases / destroy) for an in-place integer sum over ranks. */
+int pbs4d_phase_energy_ptr(pbs4d_ctx* ctx, int32_t phase, int64_t** q_dev);
+
+/* a7 again, from the (now summed) energy grid: refreshes the phase dose kept by the context. */
+int pbs4d_finalize_phase_dose(pbs4d_ctx* ctx, int32_t phase, double per_protons);
+
+/* a8 alone: zero the accumulators of every eligible source phase (DVF to ref_phase + a dose) and push those whose
+ * bit is set in src_mask.  stats->subvoxels counts the pushed phases only. */
+int pbs4d_accumulate_push(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                          const float* const* phase_dose_dev, uint32_t src_mask, pbs4d_acc_stats* stats);
+
+/* Device pointers to the context's own int64 E and M sums [z][y][x] of one eligible source phase (valid as above). */
+int pbs4d_accumulator_ptrs(pbs4d_ctx* ctx, int32_t src_phase, int64_t** e_dev, int64_t** m_dev);
+
+/* a9 alone over every eligible source phase (all of them must have been pushed or received). */
+int pbs4d_accumulate_finalize(pbs4d_ctx* ctx, int32_t ref_phase, const float* const* phase_dose_dev,
+                              float* dose4d_dev, pbs4d_acc_stats* stats);
+
+/* Whole path with HOST buffers (copies inside): set_plan_spots + simulate_delivery first (host, milliseconds) -- the
+ * sub-plans say which breathing phases receive beam; then, for those phases and the reference phase only, CT upload +
+ * HU -> density, DVF upload (on a copy stream, underneath the transport), mc_dose_phases, accumulate_subvoxel and
+ * the copy of the 4D dose to dose4d_host.  CTs and DVFs of phases that receive no beam (gating) are never touched.
+ * hu_host[p] (all non-NULL), disp_host[p] (NULL = no DVF for p).  histories_run, h2d_bytes (bytes actually copied host ->
+ * device), seconds ([4]: delivery simulation, upload + density enqueue, transport, accumulate + D2H; wall times) are
+ * optional.  Afterwards the context holds densities and doses of the active phases only. */
 int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_host,
                         const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts,
                         const pbs4d_grid* dvf_grid, const float* const* disp_host, int32_t ref_phase,
                         int32_t n_fields, const pbs4d_field* fields, int64_t n_spots, const pbs4d_spot* spots,
                         const pbs4d_delivery_params* prm, uint64_t total_histories, uint64_t seed,
                         int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
-                        double* seconds);
+                        uint64_t* h2d_bytes, double* seconds);
 
 /* ---- dose-interpolation method (DIM), the paper's second accumulation method (Eq. 3; "Input
  * options allowed the user to choose both the accumulation method and the voxel-subdivision scale n").

@@ -287,3 +287,39 @@ def build_dvf(info, delta):
     if rc != 0:
         raise ValueError(f"orc_build_dvf: error {rc}")
     return rf, disp
+
+
+class TrialSpec(C.Structure):
+    """orc_trial_spec (orc.h): distributions of the uncertainty trials, PAPER.md:53-65"""
+    _fields_ = [("seed", C.c_uint64), ("n_trials", C.c_int32), ("n_cycles", C.c_int32), ("period_lo_ns", C.c_int64),
+                ("period_hi_ns", C.c_int64), ("period_step_ns", C.c_int64), ("period_sigma_ns", C.c_int64),
+                ("discard_sigma_ns", C.c_int64), ("flat_top_sigma_ns", C.c_int64), ("spot_switch_sigma_ns", C.c_int64),
+                ("layer_switch_sigma_ns", C.c_int64), ("spill_protons_sigma", C.c_int64),
+                ("protons_per_s_sigma", C.c_int64)]
+
+
+def sample_trial(spec, trial, n_fields, prm, cycle_period_ns=None, discard_ns=0, spill_protons_max=0, flat_top_ns=0,
+                 spot_switch_fixed_ns=0, layer_switch_ns=None, max_protons_per_paint=0):
+    """U0-U5 for one trial.  spec: dict of TrialSpec fields.  Returns dict(start_phase, prm (DELIV_DT record), ext
+    (keyword arguments for simulate_delivery_ext))."""
+    sp = TrialSpec(**spec)
+    p = np.ascontiguousarray(prm, DELIV_DT)
+    lsw = None if layer_switch_ns is None else np.ascontiguousarray(layer_switch_ns, np.int64)
+    x = DeliveryExt(0, None, int(discard_ns), int(spill_protons_max), int(flat_top_ns), int(spot_switch_fixed_ns),
+                    0 if lsw is None else len(lsw), None if lsw is None else lsw.ctypes.data, int(max_protons_per_paint))
+    start = np.zeros(n_fields, np.int32)
+    cyc = np.zeros(max(sp.n_cycles, 1), np.int64)
+    lsw_out = np.zeros(max(1, 0 if lsw is None else len(lsw)), np.int64)
+    p_out = np.zeros(1, DELIV_DT)
+    x_out = DeliveryExt()
+    lib().orc_sample_trial.restype = C.c_int
+    rc = lib().orc_sample_trial(C.byref(sp), C.c_int32(trial), C.c_int32(n_fields), _p(p), C.byref(x), _p(start), _p(cyc),
+                                _p(lsw_out), _p(p_out), C.byref(x_out))
+    if rc != 0:
+        raise ValueError(f"orc_sample_trial: error {rc}")
+    ext = dict(cycle_period_ns=cyc[:sp.n_cycles].copy() if sp.n_cycles > 0 else None, discard_ns=x_out.discard_ns,
+               spill_protons_max=x_out.spill_protons_max, flat_top_ns=x_out.flat_top_ns,
+               spot_switch_fixed_ns=x_out.spot_switch_fixed_ns,
+               layer_switch_ns=None if lsw is None else lsw_out[:len(lsw)].copy(),
+               max_protons_per_paint=x_out.max_protons_per_paint)
+    return dict(start_phase=start, prm=p_out, ext=ext)

@@ -7,7 +7,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["orc_physics.c", "orc_transport.c", "orc_delivery.c", "orc_accumulate.c", "orc_dim.c", "orc_dvf.c"]
+SOURCES = ["orc_physics.c", "orc_transport.c", "orc_delivery.c", "orc_accumulate.c", "orc_dim.c", "orc_dvf.c", "orc_trials.c"]
 LIB = os.path.join(HERE, "liborc.so")
 
 

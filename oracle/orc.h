@@ -73,6 +73,23 @@ int64_t orc_simulate_delivery_ext(int32_t n_fields, const orc_field* fields, int
                                   orc_segment* segs, int64_t max_segs, int64_t* total_time_ns,
                                   int64_t* dropped_protons, int64_t* n_fills);
 
+/* ---- uncertainty trials (steps U0-U5 in orc_trials.c) ---- */
+typedef struct {
+    uint64_t seed;
+    int32_t  n_trials, n_cycles;                  /* trials; breathing cycles sampled per trial (the last repeats) */
+    int64_t  period_lo_ns, period_hi_ns, period_step_ns;   /* mean period ~ U{lo, lo + step, ... <= hi}; lo = 0: fixed */
+    int64_t  period_sigma_ns;                     /* per-cycle period ~ N(mean, sigma) */
+    int64_t  discard_sigma_ns, flat_top_sigma_ns, spot_switch_sigma_ns, layer_switch_sigma_ns;
+    int64_t  spill_protons_sigma, protons_per_s_sigma;     /* 1-sigma of the synchrotron parameters; 0 = fixed */
+} orc_trial_spec;
+
+/* Sample trial `trial`: start_phase[n_fields], cycle_period_ns[spec->n_cycles], layer_switch_ns[ext->n_layer_switch]
+ * (caller's arrays); prm_out / ext_out = copies of prm / ext with the sampled values, pointing into those arrays. */
+int orc_sample_trial(const orc_trial_spec* spec, int32_t trial, int32_t n_fields,
+                     const orc_delivery_params* prm, const orc_delivery_ext* ext,
+                     int32_t* start_phase, int64_t* cycle_period_ns, int64_t* layer_switch_ns,
+                     orc_delivery_params* prm_out, orc_delivery_ext* ext_out);
+
 /* ---- transport (T1-T12) ---- */
 #define ORC_NO_MCS       1u   /* pin switch: no Highland deflection        */
 #define ORC_NO_STRAGGLE  2u   /* pin switch: no Bohr straggling            */

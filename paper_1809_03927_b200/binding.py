@@ -33,7 +33,9 @@ EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_ph
            "pbs4d_mc_dose_phase", "pbs4d_mc_dose_phases", "pbs4d_get_phase_energy", "pbs4d_accumulate_subvoxel", "pbs4d_get_accumulators",
            "pbs4d_run_plan_host", "pbs4d_simulate_delivery_host", "pbs4d_roofline_probe",
            "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim", "pbs4d_simulate_delivery_ext", "pbs4d_simulate_delivery_ext_host",
-           "pbs4d_build_dvf"]
+           "pbs4d_build_dvf", "pbs4d_shard_window", "pbs4d_set_shard", "pbs4d_phase_energy_ptr",
+           "pbs4d_finalize_phase_dose", "pbs4d_accumulate_push", "pbs4d_accumulator_ptrs", "pbs4d_accumulate_finalize",
+           "pbs4d_sample_delivery_trial", "pbs4d_simulate_delivery_trial", "pbs4d_run_trials"]
 
 
 class PhaseLists(C.Structure):
@@ -57,6 +59,23 @@ def make_delivery_ext(cycle_period_ns=None, discard_ns=0, spill_protons_max=0, f
                     int(spill_protons_max), int(flat_top_ns), int(spot_switch_fixed_ns),
                     0 if lsw is None else len(lsw), None if lsw is None else lsw.ctypes.data, int(max_protons_per_paint))
     return x, (cyc, lsw)
+
+
+class TrialSpec(C.Structure):
+    """pbs4d_trial_spec: distributions of the uncertainty trials"""
+    _fields_ = [("seed", C.c_uint64), ("n_trials", C.c_int32), ("n_cycles", C.c_int32), ("period_lo_ns", C.c_int64),
+                ("period_hi_ns", C.c_int64), ("period_step_ns", C.c_int64), ("period_sigma_ns", C.c_int64),
+                ("discard_sigma_ns", C.c_int64), ("flat_top_sigma_ns", C.c_int64), ("spot_switch_sigma_ns", C.c_int64),
+                ("layer_switch_sigma_ns", C.c_int64), ("spill_protons_sigma", C.c_int64),
+                ("protons_per_s_sigma", C.c_int64)]
+
+
+class TrialResult(C.Structure):
+    _fields_ = [("histories", C.c_uint64), ("delivery_ns", C.c_int64), ("fills", C.c_int64), ("phases_run", C.c_int32),
+                ("pad", C.c_int32), ("transport_ms", C.c_float), ("accumulate_ms", C.c_float)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_ if n != "pad"}
 
 
 class McStats(C.Structure):
@@ -106,6 +125,47 @@ def _ptr_array(tensors):
     for i, t in enumerate(tensors):
         arr[i] = None if t is None else t.data_ptr()
     return arr
+
+
+def shard_window(n_hist, rank, world):
+    """Device-free: (begin, count) of rank's slice of n_hist histories (pbs4d_shard_window)."""
+    b, c = C.c_int64(0), C.c_int64(0)
+    rc = load().pbs4d_shard_window(C.c_int64(int(n_hist)), C.c_int32(int(rank)), C.c_int32(int(world)), C.byref(b),
+                                   C.byref(c))
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_shard_window: error {rc}")
+    return int(b.value), int(c.value)
+
+
+class _DevView:
+    """a device buffer owned by the context, exposed through __cuda_array_interface__ (no copy)"""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 2, "strides": None}
+
+
+def sample_delivery_trial(spec, trial, n_fields, prm, **ext_kw):
+    """Device-free: pbs4d_sample_delivery_trial.  spec: dict of TrialSpec fields.  Returns dict(start_phase, prm (DELIV_DT
+    record), ext (keyword arguments of simulate_delivery_ext*))."""
+    sp = TrialSpec(**spec)
+    p = np.ascontiguousarray(prm, DELIV_DT)
+    x, keep = make_delivery_ext(**ext_kw)
+    start = np.zeros(n_fields, np.int32)
+    cyc = np.zeros(max(sp.n_cycles, 1), np.int64)
+    lsw = np.zeros(max(x.n_layer_switch, 1), np.int64)
+    p_out = np.zeros(1, DELIV_DT)
+    x_out = DeliveryExt()
+    rc = load().pbs4d_sample_delivery_trial(C.byref(sp), C.c_int32(trial), C.c_int32(n_fields), _np(p), C.byref(x),
+                                            _np(start), _np(cyc), _np(lsw), _np(p_out), C.byref(x_out))
+    if rc != 0:
+        raise RuntimeError(f"pbs4d_sample_delivery_trial: error {rc}")
+    ext = dict(cycle_period_ns=cyc[:sp.n_cycles].copy() if sp.n_cycles > 0 else None, discard_ns=x_out.discard_ns,
+               spill_protons_max=x_out.spill_protons_max, flat_top_ns=x_out.flat_top_ns,
+               spot_switch_fixed_ns=x_out.spot_switch_fixed_ns,
+               layer_switch_ns=lsw[:x.n_layer_switch].copy() if x.n_layer_switch > 0 and x.layer_switch_ns else None,
+               max_protons_per_paint=x_out.max_protons_per_paint)
+    return dict(start_phase=start, prm=p_out, ext=ext)
 
 
 def simulate_delivery_host(fields, spots, prm, total_histories):
@@ -253,6 +313,36 @@ class Context:
         return dict(segments=segs, field_time_ns=times, dropped_protons=int(out.dropped_protons),
                     fixed_shift=int(out.fixed_shift), fills=int(fills.value))
 
+    # ---- uncertainty trials ----
+    def simulate_delivery_trial(self, spec, trial, prm, total_histories, **ext_kw):
+        sp = TrialSpec(**spec)
+        p = np.ascontiguousarray(prm, DELIV_DT)
+        x, keep = make_delivery_ext(**ext_kw)
+        out = PhaseLists(); fills = C.c_int64(0)
+        self._check(self.lib.pbs4d_simulate_delivery_trial(self.h, C.byref(sp), C.c_int32(trial), _np(p), C.byref(x),
+                                                           C.c_uint64(int(total_histories)), C.byref(out),
+                                                           C.byref(fills)))
+        segs = np.zeros(out.n_segments, SEG_DT)
+        if out.n_segments:
+            C.memmove(segs.ctypes.data, out.segments, segs.nbytes)
+        times = np.array([out.field_time_ns[i] for i in range(out.n_fields)], np.int64)
+        return dict(segments=segs, field_time_ns=times, dropped_protons=int(out.dropped_protons),
+                    fixed_shift=int(out.fixed_shift), fills=int(fills.value))
+
+    def run_trials(self, spec, first, count, prm, total_histories, seed, ref_phase, ns_xyz, **ext_kw):
+        """-> (list of `count` 4D-dose tensors, list of per-trial result dicts)"""
+        t = self.torch
+        sp = TrialSpec(**spec)
+        p = np.ascontiguousarray(prm, DELIV_DT)
+        x, keep = make_delivery_ext(**ext_kw)
+        outs = [t.empty(self.dose_shape, dtype=t.float32, device=self.device) for _ in range(count)]
+        res = (TrialResult * count)()
+        self._check(self.lib.pbs4d_run_trials(self.h, C.byref(sp), C.c_int32(first), C.c_int32(count), _np(p),
+                                              C.byref(x), C.c_uint64(int(total_histories)), C.c_uint64(int(seed)),
+                                              C.c_int32(ref_phase), C.c_int32(ns_xyz[0]), C.c_int32(ns_xyz[1]),
+                                              C.c_int32(ns_xyz[2]), _ptr_array(outs), res))
+        return outs, [r.as_dict() for r in res]
+
     # ---- a4-a7 ----
     def mc_dose_phase(self, phase, seed, per_protons=0.0, want_dose=True, want_rho=False):
         t = self.torch
@@ -275,6 +365,49 @@ class Context:
         self._check(self.lib.pbs4d_mc_dose_phases(self.h, C.c_int32(n), arr, C.c_uint64(int(seed)),
                                                   C.c_double(float(per_protons)), st, C.byref(ms)))
         return [s.as_dict() for s in st], float(ms.value)
+
+    # ---- sharding over GPUs (one context per rank) ----
+    def set_shard(self, rank, world):
+        self._check(self.lib.pbs4d_set_shard(self.h, C.c_int32(int(rank)), C.c_int32(int(world))))
+
+    def phase_energy_view(self, phase):
+        """int64 tensor aliasing the context's energy grid of `phase` (for an in-place all_reduce)"""
+        q = C.c_void_p()
+        self._check(self.lib.pbs4d_phase_energy_ptr(self.h, C.c_int32(phase), C.byref(q)))
+        return self.torch.as_tensor(_DevView(q.value, self.dose_shape, "<i8"), device=self.device)
+
+    def finalize_phase_dose(self, phase, per_protons=0.0):
+        self._check(self.lib.pbs4d_finalize_phase_dose(self.h, C.c_int32(phase), C.c_double(float(per_protons))))
+
+    def accumulate_push(self, ref_phase, ns_xyz, src_mask, phase_doses=None):
+        t = self.torch
+        ptrs = None
+        if phase_doses is not None:
+            ptrs = _ptr_array([None if d is None else self._dev(d, t.float32) for d in phase_doses])
+        st = AccStats()
+        self._check(self.lib.pbs4d_accumulate_push(self.h, C.c_int32(ref_phase), C.c_int32(ns_xyz[0]),
+                                                   C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), ptrs,
+                                                   C.c_uint32(int(src_mask)), C.byref(st)))
+        return st.as_dict()
+
+    def accumulator_views(self, src_phase):
+        """(E, M) int64 tensors aliasing the context's sums of one source phase"""
+        e, m = C.c_void_p(), C.c_void_p()
+        self._check(self.lib.pbs4d_accumulator_ptrs(self.h, C.c_int32(src_phase), C.byref(e), C.byref(m)))
+        t = self.torch
+        return (t.as_tensor(_DevView(e.value, self.dose_shape, "<i8"), device=self.device),
+                t.as_tensor(_DevView(m.value, self.dose_shape, "<i8"), device=self.device))
+
+    def accumulate_finalize(self, ref_phase, phase_doses=None):
+        t = self.torch
+        out = t.empty(self.dose_shape, dtype=t.float32, device=self.device)
+        ptrs = None
+        if phase_doses is not None:
+            ptrs = _ptr_array([None if d is None else self._dev(d, t.float32) for d in phase_doses])
+        st = AccStats()
+        self._check(self.lib.pbs4d_accumulate_finalize(self.h, C.c_int32(ref_phase), ptrs, C.c_void_p(out.data_ptr()),
+                                                       C.byref(st)))
+        return out, st.as_dict()
 
     def get_phase_energy(self, phase):
         t = self.torch
@@ -341,7 +474,7 @@ class Context:
                       total_histories, seed, ns_xyz, out_host, hu_pts=(-1000.0, 0.0, 1000.0),
                       rho_pts=(0.001, 1.0, 1.6)):
         """hu_host: list of int16 numpy arrays (or pinned CPU tensors' numpy views); disp_host: list (None = no DVF);
-        out_host: float32 numpy array [z,y,x] written in place.  Returns (histories_run, seconds[4])."""
+        out_host: float32 numpy array [z,y,x] written in place.  Returns (histories_run, seconds[4], h2d_bytes)."""
         ct = np.ascontiguousarray(ct_grid, GRID_DT)
         dg = None if dose_grid is None else np.ascontiguousarray(dose_grid, GRID_DT)
         vg = None if dvf_grid is None else np.ascontiguousarray(dvf_grid, GRID_DT)
@@ -355,12 +488,15 @@ class Context:
         s = np.ascontiguousarray(spots, SPOT_DT)
         p = np.ascontiguousarray(prm, DELIV_DT)
         run = C.c_uint64(0)
+        h2d = C.c_uint64(0)
         secs = (C.c_double * 4)()
         self._check(self.lib.pbs4d_run_plan_host(
             self.h, C.c_int32(n), _np(ct), hu_ptrs, None if dg is None else _np(dg), C.c_int32(len(hp)), _np(hp),
             _np(rp), None if vg is None else _np(vg), dp, C.c_int32(ref_phase), C.c_int32(len(f)), _np(f),
             C.c_int64(len(s)), _np(s), _np(p), C.c_uint64(int(total_histories)), C.c_uint64(int(seed)),
-            C.c_int32(ns_xyz[0]), C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), _np(out_host), C.byref(run), secs))
+            C.c_int32(ns_xyz[0]), C.c_int32(ns_xyz[1]), C.c_int32(ns_xyz[2]), _np(out_host), C.byref(run), C.byref(h2d),
+            secs))
         g = ct if dg is None else dg
         self.dose_shape = (int(g["nz"][0]), int(g["ny"][0]), int(g["nx"][0]))
-        return int(run.value), list(secs)
+        self.n_phases = n
+        return int(run.value), list(secs), int(h2d.value)

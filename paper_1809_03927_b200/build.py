@@ -14,7 +14,7 @@ LIB = os.path.join(HERE, "libpbs4d.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
 UNITS = [("api.cu", []), ("transport.cu", []), ("grids.cu", ["-fmad=false"]), ("accumulate.cu", ["-fmad=false"]), ("roofline.cu", []),
-         ("delivery.cpp", []), ("tables.cpp", [])]
+         ("delivery.cpp", []), ("tables.cpp", []), ("trials.cpp", [])]
 
 
 def _sources():

@@ -17,6 +17,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 
 namespace pbs4d {
 
@@ -48,18 +49,52 @@ __device__ __forceinline__ float lerp_rn(float A, float B, float w)
     return __fadd_rn(A, __fmul_rn(w, __fsub_rn(B, A)));
 }
 
-// A4: ix = floorf((q - o) / h) with the IEEE quotient, inside iff 0 <= ix < n.  The division is replaced by a
-// multiplication with inv_h = RN(1/h): y = RN(d inv_h) differs from the IEEE quotient RN(d / h) by at most
-// (2^-23 + 2^-24) |y|, so both have the same floor unless y lies within that distance of an integer; in that (rare)
-// case the quotient itself is evaluated.  The result is bit-identical to the plain definition.
-__device__ __forceinline__ float floor_quotient(float d, float h, float inv_h)
+// A4: ix = floorf((q - o) / h) with the IEEE quotient Q = RN(RN(q - o) / h), inside iff 0 <= ix < n.
+// Fast path (FMA/ALU pipes only, no division, no conversion instruction, no call):
+//   y = fma(q, inv_h, c),  inv_h = RN(1/h),  c = RN(-o inv_h - 0.5)      ~  Q - 0.5
+//   t = y + 1.5 2^23  rounds y to the nearest integer r = t - 1.5 2^23 (exact for |y| < 2^22), and r is also the
+//   difference of the bit patterns of t and 1.5 2^23.  Unless Q lies close to an integer, floor(Q) = r.
+// |y - (Q - 0.5)| <= 2^-24 (|Q| + |q inv_h| + |c| + |y|) + ulp(c)/2: the rounding of q - o that the contract
+// prescribes is a relative 2^-24 on Q, inv_h carries a relative 2^-24, c and y one rounding each.  The launcher
+// turns this into a per-axis tolerance tol = 4e-7 (n + 2 + 2 |o| / h); when fr = y - r is within tol of +-0.5, Q is
+// that close to an integer and the decision is taken exactly (exact_floor).  For |y| >= 2^22 (and +-Inf) the integer
+// comes out >= 2^22 - 1 or negative, i.e. outside every grid the fast path is used for (the launcher passes
+// tol = +Inf -- always exact -- when a reference dimension exceeds 4e6); NaN fails the comparison and goes exact.
+constexpr float kMagic     = 12582912.0f;          // 1.5 * 2^23
+constexpr int   kMagicBits = 0x4B400000;
+
+__device__ __forceinline__ bool fast_floor(float q, float inv_h, float c, float half_minus_tol, int& ix)
 {
-    const float y  = __fmul_rn(d, inv_h);
-    float fl = floorf(y);
-    const float fr  = __fsub_rn(y, fl);
-    const float tol = __fmul_rn(fabsf(y), 4.0e-7f);
-    if (!(fr >= tol && fr <= __fsub_rn(1.0f, tol))) fl = floorf(__fdiv_rn(d, h));      // also catches NaN/Inf
-    return fl;
+    const float y  = __fmaf_rn(q, inv_h, c);
+    const float t  = __fadd_rn(y, kMagic);
+    const float fr = __fsub_rn(y, __fsub_rn(t, kMagic));
+    ix = __float_as_int(t) - kMagicBits;
+    return !(fabsf(fr) <= half_minus_tol);         // true: Q is too close to an integer (or NaN) -> exact_floor
+}
+
+// Exact floorf(RN(e / h)) for e = RN(q - o), decided without a division instruction or subroutine (the kernel's
+// inner loop stays free of calls).  yq = RN(e inv_h) is within 2^-23 |yq| of Q = RN(e / h); k = the integer nearest
+// to yq.  If yq is not that close to k, floor(Q) = floor(yq).  Otherwise Q >= k  <=>  e / h >= m, where m is the
+// midpoint between k and the float below it (a tie rounds to k, whose significand is even for every integer
+// k < 2^23)  <=>  (double)e >= m (double)h, and that product is exact in double (m has <= 26, h 24 significant bits).
+// Returns the index if it is inside [0, n), else -1.  (e / h underflowing to -0 for e < 0 would be floored to -0 =
+// "inside" by the definition; that needs |e| < 2^-149 h and cannot occur for coordinates in mm.)
+__device__ __forceinline__ int exact_floor(float e, float h, float inv_h, int n)
+{
+    const float yq = __fmul_rn(e, inv_h);
+    if (!(fabsf(yq) < 4194304.0f)) return -1;                          // beyond any grid (or NaN)
+    const float k = rintf(yq);
+    int fl;
+    if (fabsf(__fsub_rn(yq, k)) > __fmul_rn(fabsf(yq), 3.0e-7f) + 1.0e-30f) fl = (int)floorf(yq);
+    else if (k < 1.0f) fl = (k == 0.0f && e >= 0.0f) ? 0 : -1;
+    else {
+        const int kb = __float_as_int(k);
+        const int ex = (kb >> 23) - 127;                               // k = 2^ex * 1.f
+        const int half_gap_exp = ex - 24 - ((kb & 0x7FFFFF) == 0 ? 1 : 0);      // half the gap to the float below k
+        const double m = __dsub_rn((double)k, __hiloint2double((1023 + half_gap_exp) << 20, 0));
+        fl = ((double)e >= __dmul_rn(m, (double)h)) ? (int)k : (int)k - 1;
+    }
+    return (unsigned)fl < (unsigned)n ? fl : -1;
 }
 
 // planar [3][N] displacement field -> one float4 {ux, uy, uz, 0} per DVF node, so that a trilinear corner is one
@@ -80,6 +115,8 @@ struct PushParams {
     const float* __restrict__ rho;
     const float4* __restrict__ U;            // interleaved DVF
     float inv_hrx, inv_hry, inv_hrz;         // RN(1 / h) of the reference grid
+    float cx, cy, cz;                        // RN(-o inv_h - 0.5) per axis (fast_floor)
+    float htx, hty, htz;                     // 0.5 - tol per axis (fast_floor)
     int nsx, nsy, nsz;
     int chunk_z;                             // source voxels along z handled by one thread (<= kChunkZMax)
     unsigned long long* E;
@@ -87,6 +124,37 @@ struct PushParams {
     AccCounters* counters;
 };
 
+// the four DVF nodes (x0|x0+1, y0|y0+1) of one z-node that a subvoxel column interpolates between
+struct Quad { float4 a00, a01, a10, a11; };
+
+__device__ __forceinline__ Quad load_quad(const float4* __restrict__ p, int dx1, int sy1)
+{
+    Quad q;
+    q.a00 = __ldg(p); q.a01 = __ldg(p + dx1); q.a10 = __ldg(p + sy1); q.a11 = __ldg(p + sy1 + dx1);
+    return q;
+}
+
+// x- then y-interpolation of the three displacement components at one z-node (A3: 2 + 1 of the 7 lerps)
+__device__ __forceinline__ void bilerp3(const Quad& q, float wx, float wy, float& cx, float& cy, float& cz)
+{
+    cx = lerp_rn(lerp_rn(q.a00.x, q.a01.x, wx), lerp_rn(q.a10.x, q.a11.x, wx), wy);
+    cy = lerp_rn(lerp_rn(q.a00.y, q.a01.y, wx), lerp_rn(q.a10.y, q.a11.y, wx), wy);
+    cz = lerp_rn(lerp_rn(q.a00.z, q.a01.z, wx), lerp_rn(q.a10.z, q.a11.z, wx), wy);
+}
+
+// Thread = a column of chunk_z source voxels along z at (i, j); CTA = 32 x 4 such columns.
+// Loop nest: subvoxel (b, a) of the column outside, ALL its z-subvoxels inside.  The integer sums do not depend on
+// the visiting order, so the nest is arranged for reuse:
+//   * the z-sequence of DVF cells is the same for every thread of the CTA (the z-axis map lives in shared memory), so
+//     the "new z-cell" branch is warp-uniform;
+//   * the x- and y-lerps (A3) are evaluated once per z-NODE of the column: walking up, the upper node of one cell is
+//     the lower node of the next, and the difference c1 - c0 of the z-lerp is formed once per cell;
+//   * per subvoxel only the z-lerp (mul, add per component), q = p + u, q - o, the product with RN(1/h) and the
+//     floor (fast_floor) remain -- all on the FMA/ALU pipes, no conversion or division instruction;
+//   * consecutive subvoxels of a voxel that land in the same reference voxel are merged into one pair of
+//     red.global.add.u64; drop counters are derived from per-column counts, not per subvoxel.
+// Each value is produced by exactly the operations of the contract, so the
+// result stays bit-identical to the oracle.
 __global__ void __launch_bounds__(kTileX * kTileY)
 emtm_push_kernel(const __grid_constant__ PushParams P)
 {
@@ -108,9 +176,14 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         else if (e < n_x + n_y)
             s_map[e] = axis_map(P.src.oy, P.src.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
                                 P.dvf.oy, P.dvf.hy, P.dvf.ny);
-        else
-            sz[e - n_x - n_y] = axis_map(P.src.oz, P.src.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
-                                         P.dvf.oz, P.dvf.hz, P.dvf.nz);
+        else {
+            AxisEntry m = axis_map(P.src.oz, P.src.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
+                                   P.dvf.oz, P.dvf.hz, P.dvf.nz);
+            // a z-subvoxel outside the DVF extent is dropped (A3): a NaN coordinate sends it through exact_floor,
+            // which returns "outside", so the inner loop needs no per-subvoxel flag test
+            if (!(m.flags & 2)) m.p = __int_as_float(0x7fc00000);
+            sz[e - n_x - n_y] = m;
+        }
     }
     const bool mine = i < P.src.nx && j < P.src.ny;
     if (mine) {
@@ -131,73 +204,79 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         const int dx1 = dnx > 1 ? 1 : 0;                 // upper x node = lower + 1 unless the DVF grid is 1 node wide
         const float orx = P.ref.ox, ory = P.ref.oy, orz = P.ref.oz, hrx = P.ref.hx, hry = P.ref.hy, hrz = P.ref.hz;
         const float ihx = P.inv_hrx, ihy = P.inv_hry, ihz = P.inv_hrz;
-        const float fnx = (float)P.ref.nx, fny = (float)P.ref.ny, fnz = (float)P.ref.nz;
-        const int rnx = P.ref.nx, rny = P.ref.ny;
+        const float fcx = P.cx, fcy = P.cy, fcz = P.cz, htx = P.htx, hty = P.hty, htz = P.htz;
+        const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * nsy;
-        // Loop nest: y, x outside, z INSIDE.  The integer sums do not depend on the order in which subvoxels are
-        // visited, so the nest is arranged for reuse: all subvoxels of a (b, a) column that fall into the same DVF
-        // z-cell share the 8 corner vectors and the 6 x- and y-lerps per component (A3); only the z-lerp, q = p + u
-        // and the destination index are evaluated per subvoxel.  Each value is computed by exactly the operations
-        // of the contract, so the result stays bit-identical.
         const int sz_stride = dny * dnx;
+        int okz = 0;                                     // z-subvoxels of the column inside the DVF extent (CTA-uniform)
+        for (int s = 0; s < n_z; ++s) okz += (sz[s].flags >> 1) & 1;
+        unsigned landed = 0, eligible = 0;
         for (int b = 0; b < nsy; ++b) {
             const AxisEntry my = syl[b];
             const int sy1 = (my.flags & 1) * dnx;
             for (int a = 0; a < nsx; ++a) {
                 const AxisEntry mx = sxl[a * kTileX];
-                const bool ok_xy = (mx.flags & my.flags & 2) != 0;
+                if (!(mx.flags & my.flags & 2)) continue;                         // whole column outside the DVF extent
+                eligible += (unsigned)okz;
                 const float4* __restrict__ col = P.U + my.i0 * dnx + mx.i0;       // (y0, x0) of the column, z = 0
+                int node_hi = -1;                                                 // z-node whose bilerp is held in c1*
+                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f, ddx = 0.f, ddy = 0.f, ddz = 0.f;
                 int cell_z = -1;
-                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f;
+                const AxisEntry* mzp = sz;
                 for (int kk = 0; kk < kz_n; ++kk) {
                     const longlong2 em = s_em[kk * (kTileX * kTileY) + tid];
                     const long long e_q = em.x, m_q = em.y;
-                    int run_dst = -1, run_cnt = 0;
-                    for (int c = 0; c < nsz; ++c) {
-                        const AxisEntry mz = sz[kk * nsz + c];
-                        if (mz.i0 != cell_z) {                                    // new DVF z-cell: corners + x/y lerps
+                    int run_dst = -1; unsigned run_cnt = 0u;
+                    for (int c = 0; c < nsz; ++c, ++mzp) {
+                        const AxisEntry mz = *mzp;
+                        if (mz.i0 != cell_z) {                                    // new DVF z-cell (warp-uniform branch)
                             cell_z = mz.i0;
-                            const float4* __restrict__ p00 = col + mz.i0 * sz_stride;
-                            const float4* __restrict__ p10 = p00 + (mz.flags & 1) * sz_stride;
-                            const float4 a000 = __ldg(p00), a001 = __ldg(p00 + dx1);
-                            const float4 a010 = __ldg(p00 + sy1), a011 = __ldg(p00 + sy1 + dx1);
-                            const float4 a100 = __ldg(p10), a101 = __ldg(p10 + dx1);
-                            const float4 a110 = __ldg(p10 + sy1), a111 = __ldg(p10 + sy1 + dx1);
-#define PBS4D_BILERP(A, B, C, D, cmp) lerp_rn(lerp_rn(A.cmp, B.cmp, mx.w), lerp_rn(C.cmp, D.cmp, mx.w), my.w)
-                            c0x = PBS4D_BILERP(a000, a001, a010, a011, x); c1x = PBS4D_BILERP(a100, a101, a110, a111, x);
-                            c0y = PBS4D_BILERP(a000, a001, a010, a011, y); c1y = PBS4D_BILERP(a100, a101, a110, a111, y);
-                            c0z = PBS4D_BILERP(a000, a001, a010, a011, z); c1z = PBS4D_BILERP(a100, a101, a110, a111, z);
-#undef PBS4D_BILERP
+                            const int hi = mz.i0 + (mz.flags & 1);
+                            if (mz.i0 == node_hi) { c0x = c1x; c0y = c1y; c0z = c1z; }
+                            else bilerp3(load_quad(col + (size_t)mz.i0 * sz_stride, dx1, sy1), mx.w, my.w, c0x, c0y, c0z);
+                            if (hi == mz.i0) { c1x = c0x; c1y = c0y; c1z = c0z; }
+                            else bilerp3(load_quad(col + (size_t)hi * sz_stride, dx1, sy1), mx.w, my.w, c1x, c1y, c1z);
+                            node_hi = hi;
+                            ddx = __fsub_rn(c1x, c0x); ddy = __fsub_rn(c1y, c0y); ddz = __fsub_rn(c1z, c0z);
                         }
-                        const bool ok = ok_xy && (mz.flags & 2);
-                        const float qx = __fadd_rn(mx.p, lerp_rn(c0x, c1x, mz.w));  // q = p + u (A4)
-                        const float qy = __fadd_rn(my.p, lerp_rn(c0y, c1y, mz.w));
-                        const float qz = __fadd_rn(mz.p, lerp_rn(c0z, c1z, mz.w));
-                        const float fx = floor_quotient(__fsub_rn(qx, orx), hrx, ihx);
-                        const float fy = floor_quotient(__fsub_rn(qy, ory), hry, ihy);
-                        const float fz = floor_quotient(__fsub_rn(qz, orz), hrz, ihz);
-                        const bool inside = fx >= 0.0f && fx < fnx && fy >= 0.0f && fy < fny && fz >= 0.0f && fz < fnz;
-                        n_dvf += ok ? 0u : 1u;
-                        n_ref += (ok && !inside) ? 1u : 0u;
-                        const int dst = (ok && inside) ? ((int)fz * rny + (int)fy) * rnx + (int)fx : -1;
+                        // z-lerp (A3), q = p + u (A4), destination index
+                        const float qx = __fadd_rn(mx.p, __fadd_rn(c0x, __fmul_rn(mz.w, ddx)));
+                        const float qy = __fadd_rn(my.p, __fadd_rn(c0y, __fmul_rn(mz.w, ddy)));
+                        const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, ddz)));
+                        int ix, iy, iz;
+                        const bool near_x = fast_floor(qx, ihx, fcx, htx, ix);
+                        const bool near_y = fast_floor(qy, ihy, fcy, hty, iy);
+                        const bool near_z = fast_floor(qz, ihz, fcz, htz, iz);
+                        if (near_x | near_y | near_z) {                           // rare: decide exactly
+                            ix = exact_floor(__fsub_rn(qx, orx), hrx, ihx, rnx);
+                            iy = exact_floor(__fsub_rn(qy, ory), hry, ihy, rny);
+                            iz = exact_floor(__fsub_rn(qz, orz), hrz, ihz, rnz);
+                        }
+                        const bool outside = ((unsigned)ix >= (unsigned)rnx) | ((unsigned)iy >= (unsigned)rny) |
+                                             ((unsigned)iz >= (unsigned)rnz);
+                        const int dst = outside ? -1 : (iz * rny + iy) * rnx + ix;
                         // merge consecutive subvoxels of the voxel that land in the same reference voxel
                         if (dst != run_dst) {
                             if (run_dst >= 0) {
-                                atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
-                                atomicAdd(P.M + run_dst, (unsigned long long)(run_cnt * m_q));
+                                atomicAdd(P.E + run_dst, (unsigned long long)e_q * run_cnt);
+                                atomicAdd(P.M + run_dst, (unsigned long long)m_q * run_cnt);
+                                landed += run_cnt;
                             }
-                            run_dst = dst; run_cnt = 0;
+                            run_dst = dst; run_cnt = 0u;
                         }
-                        run_cnt += 1;
+                        run_cnt += 1u;
                     }
                     if (run_dst >= 0) {
-                        atomicAdd(P.E + run_dst, (unsigned long long)(run_cnt * e_q));
-                        atomicAdd(P.M + run_dst, (unsigned long long)(run_cnt * m_q));
+                        atomicAdd(P.E + run_dst, (unsigned long long)e_q * run_cnt);
+                        atomicAdd(P.M + run_dst, (unsigned long long)m_q * run_cnt);
+                        landed += run_cnt;
                     }
                 }
             }
         }
+        n_dvf = (unsigned)(nsx * nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
+        n_ref = eligible - landed;                        // mapped outside the reference grid (A4)
     }
     // drop counters: warp-reduce, one atomic per warp
 #pragma unroll
@@ -433,10 +512,17 @@ dim_final_kernel(pbs4d_grid ref, const double* __restrict__ acc, const unsigned 
 
 }  // namespace
 
+cudaError_t configure_accumulate(void)
+{
+    // the push kernel's axis maps + per-voxel (e_q, m_q) stage need up to 57 KB of dynamic shared memory at 64
+    // subvoxels per axis.  A per-device attribute: pbs4d_create calls this for every context.
+    return cudaFuncSetAttribute(emtm_push_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+}
+
 void launch_dvf_interleave(const pbs4d_grid& g, const float* disp_planar, float* out4, cudaStream_t st)
 {
     const size_t n = (size_t)g.nx * g.ny * g.nz;
-    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 16);
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)sm_count_of_current_device() * 16);
     dvf_interleave_kernel<<<blocks, 256, 0, st>>>(n, disp_planar, disp_planar + n, disp_planar + 2 * n,
                                                   reinterpret_cast<float4*>(out4));
 }
@@ -449,22 +535,26 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     P.src = src; P.dvf = dvf_grid; P.ref = ref; P.dose = dose; P.rho = rho;
     P.U = reinterpret_cast<const float4*>(disp4);
     P.inv_hrx = 1.0f / ref.hx; P.inv_hry = 1.0f / ref.hy; P.inv_hrz = 1.0f / ref.hz;
+    // fast_floor constants per axis: c = RN(-o inv_h - 0.5); tolerance 4e-7 (n + 2 + 2 |o| / h) (see fast_floor);
+    // 0.5 - tol < 0 (always exact) for grids too long for the 2^22 range of the bit trick
+    auto cst = [](float o, float inv_h) { return (float)(-(double)o * (double)inv_h - 0.5); };
+    auto hmt = [](int n, float o, float h) {
+        const double tol = 4.0e-7 * ((double)n + 2.0 + 2.0 * std::fabs((double)o) / (double)h);
+        return (n <= 4000000 && tol < 0.25) ? (float)(0.5 - tol) : -1.0f;
+    };
+    P.cx = cst(ref.ox, P.inv_hrx); P.cy = cst(ref.oy, P.inv_hry); P.cz = cst(ref.oz, P.inv_hrz);
+    P.htx = hmt(ref.nx, ref.ox, ref.hx); P.hty = hmt(ref.ny, ref.oy, ref.hy); P.htz = hmt(ref.nz, ref.oz, ref.hz);
     P.nsx = nsx; P.nsy = nsy; P.nsz = nsz;
     P.E = (unsigned long long*)E; P.M = (unsigned long long*)M; P.counters = counters;
-    // z-chunk per thread: with <= 2 subvoxels per voxel along z, neighbouring voxels share DVF z-cells and a column of
-    // 8 voxels per thread halves the x/y-lerp work and amortises the CTA prologue (measured +12 % at n = 2); with more
-    // subvoxels per voxel the sharing is already inside the voxel and longer columns only cost registers (-10 % at n = 8)
-    P.chunk_z = nsz <= 2 ? kChunkZMax : 1;
+    // z-chunk per thread: the x/y-lerps are evaluated once per z-node of a column, and the first node of a column is
+    // extra, so longer columns amortise it (and the CTA prologue); measured on config 4 (chunk 1 -> this choice):
+    // n = 4 5.09 -> 4.19 ms, n = 8 29.9 -> 27.8 ms, (2,2,5) 1.69 -> 1.45 ms per 9 phases of 128^3
+    P.chunk_z = nsz <= 2 ? kChunkZMax : (nsz <= 4 ? 4 : 2);
     dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY,
                                  (src.nz + P.chunk_z - 1) / P.chunk_z);
     const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
                         (size_t)P.chunk_z * kTileX * kTileY * sizeof(longlong2);
-    static bool configured = false;
-    if (!configured) {                                   // up to 57 KB at 64 subvoxels per axis
-        cudaFuncSetAttribute(emtm_push_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        configured = true;
-    }
-    emtm_push_kernel<<<g, b, smem, st>>>(P);
+    emtm_push_kernel<<<g, b, smem, st>>>(P);             // > 48 KB possible: configure_accumulate() opted in
 }
 
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_host,
@@ -491,7 +581,7 @@ void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_sr
 void launch_dim_init(const pbs4d_grid& ref, const float* dose_ref, double* acc, cudaStream_t st)
 {
     const size_t n = (size_t)ref.nx * ref.ny * ref.nz;
-    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 16);
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)sm_count_of_current_device() * 16);
     dim_init_kernel<<<blocks, 256, 0, st>>>(n, dose_ref, acc);
 }
 

@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <chrono>
 #include <cmath>
 #include <cstdio>
@@ -63,6 +64,7 @@ struct pbs4d_ctx {
     int32_t n_phases = 0;
     pbs4d_grid dose_grid{};
     std::vector<std::unique_ptr<DevBuf>> rho;            // [phase] fp32 on dose grid
+    std::vector<bool> rho_valid;                         // [phase] density grid filled (run_plan_host fills active phases only)
     DevBuf table;                                        // hu_pts | rho_pts
 
     // DVFs (a2)
@@ -88,6 +90,8 @@ struct pbs4d_ctx {
     std::vector<std::unique_ptr<DevBuf>> dose;           // [phase] fp32 Gy
     std::vector<bool> have_dose;
     DevBuf counters;
+    DevBuf phys_tab;                                     // per-energy physics table of the transport kernel (per context)
+    int32_t shard_rank = 0, shard_world = 1;             // history sharding (pbs4d_set_shard)
     std::vector<std::unique_ptr<DevBuf>> seg_phase;      // [phase] launch table (DevSegment[] | seg_begin[])
     std::vector<cudaStream_t> aux;                       // auxiliary streams for concurrent phase launches
     cudaStream_t copy_stream = nullptr;                  // uploads that overlap compute (run_plan_host)
@@ -115,13 +119,27 @@ int cuda_fail(pbs4d_ctx* c, cudaError_t e, const char* what)
                 std::string(what) + ": " + cudaGetErrorString(e));
 }
 
+// Nothing may throw across the C boundary: every extern "C" entry point is a function-try-block ending here.
+int on_exception(pbs4d_ctx* c) noexcept
+{
+    try { throw; }
+    catch (const std::bad_alloc&) {
+        try { if (c) c->err = "out of host memory"; } catch (...) {}
+        return PBS4D_ERR_NOMEM;
+    }
+    catch (...) {
+        try { if (c) c->err = "unexpected C++ exception"; } catch (...) {}
+        return PBS4D_ERR_ARG;
+    }
+}
+
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
 
 bool grid_ok(const pbs4d_grid* g)
 {
     return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->hx > 0.0f && g->hy > 0.0f && g->hz > 0.0f &&
            std::isfinite(g->ox) && std::isfinite(g->oy) && std::isfinite(g->oz) &&
-           (double)g->nx * g->ny * g->nz < 2.0e9;
+           g->nx <= 4000000 && g->ny <= 4000000 && g->nz <= 4000000 && (double)g->nx * g->ny * g->nz < 2.0e9;
 }
 
 void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
@@ -140,6 +158,7 @@ void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
     for (auto& d : ctx->dvf_pull) { d.set = false; d.ref = -1; }
     ctx->have_dose.assign(n_phases, false);
     ctx->have_acc.assign(n_phases, false);
+    ctx->rho_valid.assign(n_phases, false);
     ctx->have_density = false;
 }
 
@@ -147,7 +166,7 @@ void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
 
 extern "C" {
 
-int pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream)
+int pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream) try
 {
     if (!out) return PBS4D_ERR_ARG;
     *out = nullptr;
@@ -158,13 +177,24 @@ int pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream)
     if (!ctx) return PBS4D_ERR_NOMEM;
     ctx->device = device;
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
-    cudaDeviceProp prop{};
-    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) ctx->sm_count = prop.multiProcessorCount;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) ctx->sm_count = sms;
+    // per-context physics table and per-device kernel attributes: uploaded / set here, checked, and ordered before
+    // any launch (the copy is synchronised; the launches of every stream come later)
+    std::vector<char> host_tab(physics_table_bytes());
+    build_physics_table_host(host_tab.data());
+    cudaError_t e = ctx->phys_tab.ensure(host_tab.size());
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->phys_tab.p, host_tab.data(), host_tab.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = configure_transport();
+    if (e == cudaSuccess) e = configure_accumulate();
+    if (e != cudaSuccess) { delete ctx; return e == cudaErrorMemoryAllocation ? PBS4D_ERR_NOMEM : PBS4D_ERR_CUDA; }
     *out = ctx;
     return PBS4D_OK;
 }
+catch (...) { return on_exception(nullptr); }
 
-void pbs4d_destroy(pbs4d_ctx* ctx)
+void pbs4d_destroy(pbs4d_ctx* ctx) try
 {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
@@ -173,11 +203,12 @@ void pbs4d_destroy(pbs4d_ctx* ctx)
     if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
     delete ctx;
 }
+catch (...) {}
 
 const char* pbs4d_last_error(const pbs4d_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_dev,
-                        const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts)
+                        const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_dev || (dose_grid && !grid_ok(dose_grid)) ||
@@ -202,12 +233,14 @@ int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, 
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(ctx->stream));
+    ctx->rho_valid.assign(n_phases, true);
     ctx->have_density = true;
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* dose_grid,
-                             const float* const* rho_dev)
+                             const float* const* rho_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (n_phases < 1 || n_phases > 32 || !grid_ok(dose_grid) || !rho_dev)
@@ -215,15 +248,25 @@ int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid*
     for (int p = 0; p < n_phases; ++p) if (!rho_dev[p]) return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: null phase");
     CU(cudaSetDevice(ctx->device));
     reset_phase_state(ctx, n_phases, *dose_grid);
+    CU(ctx->counters.ensure(sizeof(TransportCounters) * 32));
+    int* bad_dev = ctx->counters.as<int>();               // scratch word for the validation kernel
+    CU(cudaMemsetAsync(bad_dev, 0, sizeof(int), ctx->stream));
     for (int p = 0; p < n_phases; ++p) {
         CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
         CU(cudaMemcpyAsync(ctx->rho[p]->p, rho_dev[p], ctx->nvox() * sizeof(float), cudaMemcpyDeviceToDevice,
                            ctx->stream));
+        launch_validate_density(ctx->rho[p]->as<float>(), ctx->nvox(), bad_dev, ctx->stream);
     }
+    int bad = 0;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(&bad, bad_dev, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    if (bad) return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: densities must be finite and within [1e-6, 100] g/cm3");
+    ctx->rho_valid.assign(n_phases, true);
     ctx->have_density = true;
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const char* who, int32_t src_phase,
                      int32_t ref_phase, const pbs4d_grid* dvf_grid, const float* disp_dev)
@@ -246,21 +289,23 @@ static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const c
 }
 
 int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
-                  const float* disp_dev)
+                  const float* disp_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     return store_dvf(ctx, ctx->dvf, "set_dvf", src_phase, ref_phase, dvf_grid, disp_dev);
 }
+catch (...) { return on_exception(ctx); }
 
 int pbs4d_set_dvf_pull(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
-                       const float* disp_dev)
+                       const float* disp_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     return store_dvf(ctx, ctx->dvf_pull, "set_dvf_pull", src_phase, ref_phase, dvf_grid, disp_dev);
 }
+catch (...) { return on_exception(ctx); }
 
 int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fields,
-                         int64_t n_spots, const pbs4d_spot* spots)
+                         int64_t n_spots, const pbs4d_spot* spots) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (n_fields < 1 || !fields || n_spots < 1 || !spots) return fail(ctx, PBS4D_ERR_ARG, "set_plan_spots: bad argument");
@@ -281,13 +326,15 @@ int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fi
     ctx->have_delivery = false;
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
-int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags)
+int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     ctx->mc_flags = flags;
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 }  // extern "C"
 
@@ -299,15 +346,16 @@ extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_
                                            pbs4d_phase_lists* out, int64_t* n_fills);
 
 extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
-                                       pbs4d_phase_lists* out)
+                                       pbs4d_phase_lists* out) try
 {
     return pbs4d_simulate_delivery_ext(ctx, prm, nullptr, total_histories, out, nullptr);
 }
+catch (...) { return on_exception(ctx); }
 
 // ext == NULL: the base simulator; else the extended model.  Both end in the same per-phase launch tables.
 extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm,
                                            const pbs4d_delivery_ext* ext, uint64_t total_histories,
-                                           pbs4d_phase_lists* out, int64_t* n_fills)
+                                           pbs4d_phase_lists* out, int64_t* n_fills) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: null parameters");
@@ -366,6 +414,7 @@ extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_
     }
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // a4-a7: transport + scoring + finalize for one phase
@@ -375,7 +424,7 @@ constexpr int kAuxStreams = 4;
 }
 
 extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* phases, uint64_t seed, double per_protons,
-                                    pbs4d_mc_stats* stats, float* elapsed_ms)
+                                    pbs4d_mc_stats* stats, float* elapsed_ms) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: no densities (set_ct_phases)");
@@ -384,6 +433,7 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
     for (int a = 0; a < n; ++a) {
         if (phases[a] < 0 || phases[a] >= ctx->n_phases || phases[a] >= ctx->deliv_phases)
             return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phases: phase out of range");
+        if (!ctx->rho_valid[phases[a]]) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: no density grid for this phase");
         for (int b = 0; b < a; ++b)
             if (phases[b] == phases[a]) return fail(ctx, PBS4D_ERR_ARG, "mc_dose_phases: phase listed twice");
     }
@@ -431,10 +481,13 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
             guard(cudaMemcpyAsync(sb.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
                                   cudaMemcpyHostToDevice, st), "segments H2D");
             guard(cudaEventRecord(ev[2 * a], st), "record");
-            launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), sb.as<DevSegment>(),
-                             reinterpret_cast<const long long*>(sb.as<char>() + seg_bytes), (int32_t)L.segs.size(),
-                             L.n_hist, seed, ctx->mc_flags, ctx->q[phase]->as<long long>(),
-                             ctx->counters.as<TransportCounters>() + a, ctx->sm_count, st);
+            int64_t h0 = 0, hn = 0;
+            pbs4d_shard_window(L.n_hist, ctx->shard_rank, ctx->shard_world, &h0, &hn);
+            if (hn > 0)
+                launch_transport(ctx->dose_grid, ctx->rho[phase]->as<float>(), sb.as<DevSegment>(),
+                                 reinterpret_cast<const long long*>(sb.as<char>() + seg_bytes), (int32_t)L.segs.size(),
+                                 h0, hn, seed, ctx->mc_flags, ctx->phys_tab.p, ctx->q[phase]->as<long long>(),
+                                 ctx->counters.as<TransportCounters>() + a, ctx->sm_count, st);
         }
         guard(cudaEventRecord(ev[2 * a + 1], st), "record");
         launch_finalize_dose(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->q[phase]->as<long long>(),
@@ -468,9 +521,10 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
     destroy_events();
     return rc;
 }
+catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
-                                   float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats)
+                                   float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     const int rc = pbs4d_mc_dose_phases(ctx, 1, &phase, seed, per_protons, stats, nullptr);
@@ -481,8 +535,9 @@ extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed,
     if (dose_dev || rho_dev) CU(cudaStreamSynchronize(ctx->stream));
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
-extern "C" int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev)
+extern "C" int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (phase < 0 || phase >= ctx->n_phases || !q_dev) return fail(ctx, PBS4D_ERR_ARG, "get_phase_energy: bad argument");
@@ -492,64 +547,128 @@ extern "C" int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_
     CU(cudaStreamSynchronize(ctx->stream));
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
+
+// ------------------------------------------------------------------------------------------------------------------
+// multi-GPU history sharding (the MC was distributed amongst eight GPUs).
+// Histories are independent units with one Philox counter each, so a rank transports a contiguous slice of every
+// phase's history range; the int64 energy grids of the ranks add up to the unsharded grid bit for bit.
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_shard_window(int64_t n_hist, int32_t rank, int32_t world, int64_t* begin, int64_t* count)
+{
+    if (n_hist < 0 || world < 1 || rank < 0 || rank >= world || !begin || !count) return PBS4D_ERR_ARG;
+    const int64_t b = (int64_t)(((__int128)n_hist * rank) / world);
+    const int64_t e = (int64_t)(((__int128)n_hist * (rank + 1)) / world);
+    *begin = b; *count = e - b;
+    return PBS4D_OK;
+}
+
+extern "C" int pbs4d_set_shard(pbs4d_ctx* ctx, int32_t rank, int32_t world) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (world < 1 || rank < 0 || rank >= world) return fail(ctx, PBS4D_ERR_ARG, "set_shard: need 0 <= rank < world");
+    ctx->shard_rank = rank; ctx->shard_world = world;      // affects the mc_dose_phase(s) calls that follow only
+    return PBS4D_OK;
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_phase_energy_ptr(pbs4d_ctx* ctx, int32_t phase, int64_t** q_dev) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (phase < 0 || phase >= ctx->n_phases || !q_dev) return fail(ctx, PBS4D_ERR_ARG, "phase_energy_ptr: bad argument");
+    if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "phase_energy_ptr: mc_dose_phase not run for this phase");
+    *q_dev = ctx->q[phase]->as<int64_t>();
+    return PBS4D_OK;
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_finalize_phase_dose(pbs4d_ctx* ctx, int32_t phase, double per_protons) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (phase < 0 || phase >= ctx->n_phases) return fail(ctx, PBS4D_ERR_ARG, "finalize_phase_dose: bad argument");
+    if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "finalize_phase_dose: mc_dose_phase not run for this phase");
+    CU(cudaSetDevice(ctx->device));
+    launch_finalize_dose(ctx->dose_grid, ctx->rho[phase]->as<float>(), ctx->q[phase]->as<long long>(), ctx->fixed_shift,
+                         per_protons, ctx->dose[phase]->as<float>(), ctx->stream);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    return PBS4D_OK;
+}
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // a8-a9: subvoxel energy/mass push of every source phase with a DVF to ref_phase, then ratio + sum + mask
 // ------------------------------------------------------------------------------------------------------------------
-extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
-                                         const float* const* phase_dose_dev, float* dose4d_dev,
-                                         pbs4d_acc_stats* stats)
+namespace {
+
+// push (a8) of the source phases selected by src_mask and / or finalize (a9) over every eligible source phase.
+// Eligible = has a DVF to ref_phase and a dose.  Eligible phases outside src_mask get zeroed accumulators (ready to
+// receive another rank's sums, pbs4d_accumulator_ptrs).
+int accumulate_impl(pbs4d_ctx* ctx, const char* who, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                    const float* const* phase_dose_dev, uint32_t src_mask, bool do_push, bool do_finalize,
+                    float* dose4d_dev, pbs4d_acc_stats* stats)
 {
-    if (!ctx) return PBS4D_ERR_ARG;
-    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_subvoxel: no densities");
-    if (ref_phase < 0 || ref_phase >= ctx->n_phases || nsx < 1 || nsy < 1 || nsz < 1 || nsx > 64 || nsy > 64 ||
-        nsz > 64 || !dose4d_dev)
-        return fail(ctx, PBS4D_ERR_ARG, "accumulate_subvoxel: bad argument");
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, std::string(who) + ": no densities");
+    if (ref_phase < 0 || ref_phase >= ctx->n_phases || (do_push && (nsx < 1 || nsy < 1 || nsz < 1 || nsx > 64 ||
+        nsy > 64 || nsz > 64)) || (do_finalize && !dose4d_dev))
+        return fail(ctx, PBS4D_ERR_ARG, std::string(who) + ": bad argument");
     auto dose_of = [&](int p) -> const float* {
         if (phase_dose_dev) return phase_dose_dev[p];
         return ctx->have_dose[p] ? ctx->dose[p]->as<float>() : nullptr;
     };
-    if (!dose_of(ref_phase)) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_subvoxel: no dose for the reference phase");
+    if (!dose_of(ref_phase)) return fail(ctx, PBS4D_ERR_ORDER, std::string(who) + ": no dose for the reference phase");
     std::vector<int> src;
     for (int p = 0; p < ctx->n_phases; ++p)
         if (p != ref_phase && ctx->dvf[p].set && ctx->dvf[p].ref == ref_phase && dose_of(p)) src.push_back(p);
-    if (src.size() > 32) return fail(ctx, PBS4D_ERR_ARG, "accumulate_subvoxel: more than 32 source phases");
+    if (src.size() > 32) return fail(ctx, PBS4D_ERR_ARG, std::string(who) + ": more than 32 source phases");
     CU(cudaSetDevice(ctx->device));
     const size_t nvox = ctx->nvox();
-    CU(ctx->acc_counters.ensure(sizeof(AccCounters)));
-    CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
     EventTrio ev;                                        // destroyed on every return path
     CU(ev.create());
     cudaEvent_t e0 = ev.e[0], e1 = ev.e[1], e2 = ev.e[2];
-    std::fill(ctx->have_acc.begin(), ctx->have_acc.end(), false);
-    for (int p : src) {
-        CU(ctx->accE[p]->ensure(nvox * sizeof(long long)));
-        CU(ctx->accM[p]->ensure(nvox * sizeof(long long)));
-        CU(cudaMemsetAsync(ctx->accE[p]->p, 0, nvox * sizeof(long long), ctx->stream));
-        CU(cudaMemsetAsync(ctx->accM[p]->p, 0, nvox * sizeof(long long), ctx->stream));
+    uint64_t pushed = 0;
+    if (do_push) {
+        CU(ctx->acc_counters.ensure(sizeof(AccCounters)));
+        CU(cudaMemsetAsync(ctx->acc_counters.p, 0, sizeof(AccCounters), ctx->stream));
+        std::fill(ctx->have_acc.begin(), ctx->have_acc.end(), false);
+        for (int p : src) {
+            CU(ctx->accE[p]->ensure(nvox * sizeof(long long)));
+            CU(ctx->accM[p]->ensure(nvox * sizeof(long long)));
+            CU(cudaMemsetAsync(ctx->accE[p]->p, 0, nvox * sizeof(long long), ctx->stream));
+            CU(cudaMemsetAsync(ctx->accM[p]->p, 0, nvox * sizeof(long long), ctx->stream));
+        }
     }
     CU(cudaEventRecord(e0, ctx->stream));
-    std::vector<const long long*> Ep, Mp; std::vector<pbs4d_grid> dg;
-    for (int p : src) {
-        launch_emtm_push(ctx->dose_grid, dose_of(p), ctx->rho[p]->as<float>(), ctx->dvf[p].grid,
-                         ctx->dvf[p].disp->as<float>(), ctx->dose_grid, nsx, nsy, nsz,
-                         ctx->accE[p]->as<long long>(), ctx->accM[p]->as<long long>(),
-                         ctx->acc_counters.as<AccCounters>(), ctx->stream);
-        Ep.push_back(ctx->accE[p]->as<long long>()); Mp.push_back(ctx->accM[p]->as<long long>());
-        dg.push_back(ctx->dvf[p].grid);
-        ctx->have_acc[p] = true;
+    if (do_push) {
+        for (int p : src) {
+            ctx->have_acc[p] = true;
+            if (!((src_mask >> p) & 1u)) continue;
+            launch_emtm_push(ctx->dose_grid, dose_of(p), ctx->rho[p]->as<float>(), ctx->dvf[p].grid,
+                             ctx->dvf[p].disp->as<float>(), ctx->dose_grid, nsx, nsy, nsz,
+                             ctx->accE[p]->as<long long>(), ctx->accM[p]->as<long long>(),
+                             ctx->acc_counters.as<AccCounters>(), ctx->stream);
+            pushed += 1;
+        }
     }
     CU(cudaEventRecord(e1, ctx->stream));
-    CU(ctx->cover_flags.ensure((size_t)ctx->dose_grid.nx + ctx->dose_grid.ny + ctx->dose_grid.nz));
-    launch_emtm_finalize(ctx->dose_grid, dose_of(ref_phase), (int)src.size(), Ep.data(), Mp.data(), dg.data(),
-                         ctx->cover_flags.as<unsigned char>(), dose4d_dev, ctx->stream);
+    if (do_finalize) {
+        std::vector<const long long*> Ep, Mp; std::vector<pbs4d_grid> dg;
+        for (int p : src) {
+            if (!ctx->have_acc[p]) return fail(ctx, PBS4D_ERR_ORDER, std::string(who) + ": source phase was not pushed");
+            Ep.push_back(ctx->accE[p]->as<long long>()); Mp.push_back(ctx->accM[p]->as<long long>());
+            dg.push_back(ctx->dvf[p].grid);
+        }
+        CU(ctx->cover_flags.ensure((size_t)ctx->dose_grid.nx + ctx->dose_grid.ny + ctx->dose_grid.nz));
+        launch_emtm_finalize(ctx->dose_grid, dose_of(ref_phase), (int)src.size(), Ep.data(), Mp.data(), dg.data(),
+                             ctx->cover_flags.as<unsigned char>(), dose4d_dev, ctx->stream);
+    }
     CU(cudaEventRecord(e2, ctx->stream));
     CU(cudaGetLastError());
     AccCounters ac{};
-    CU(cudaMemcpyAsync(&ac, ctx->acc_counters.p, sizeof(ac), cudaMemcpyDeviceToHost, ctx->stream));
+    if (do_push) CU(cudaMemcpyAsync(&ac, ctx->acc_counters.p, sizeof(ac), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     if (stats) {
-        stats->subvoxels = (uint64_t)src.size() * nvox * nsx * nsy * nsz;
+        stats->subvoxels = pushed * nvox * (do_push ? (uint64_t)nsx * nsy * nsz : 0);
         stats->dropped_outside_ref = ac.dropped_ref; stats->dropped_outside_dvf = ac.dropped_dvf;
         cudaEventElapsedTime(&stats->push_ms, e0, e1);
         cudaEventElapsedTime(&stats->finalize_ms, e1, e2);
@@ -557,7 +676,50 @@ extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int3
     return PBS4D_OK;
 }
 
-extern "C" int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev)
+}  // namespace
+
+extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                                         const float* const* phase_dose_dev, float* dose4d_dev,
+                                         pbs4d_acc_stats* stats) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    return accumulate_impl(ctx, "accumulate_subvoxel", ref_phase, nsx, nsy, nsz, phase_dose_dev, 0xFFFFFFFFu, true, true,
+                           dose4d_dev, stats);
+}
+catch (...) { return on_exception(ctx); }
+
+// the two halves of accumulate_subvoxel, for runs sharded by source phase: every rank pushes the source
+// phases of its src_mask, the int64 sums are exchanged through pbs4d_accumulator_ptrs, then a9 runs on the full set
+extern "C" int pbs4d_accumulate_push(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
+                                     const float* const* phase_dose_dev, uint32_t src_mask, pbs4d_acc_stats* stats) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    return accumulate_impl(ctx, "accumulate_push", ref_phase, nsx, nsy, nsz, phase_dose_dev, src_mask, true, false,
+                           nullptr, stats);
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_accumulate_finalize(pbs4d_ctx* ctx, int32_t ref_phase, const float* const* phase_dose_dev,
+                                         float* dose4d_dev, pbs4d_acc_stats* stats) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    return accumulate_impl(ctx, "accumulate_finalize", ref_phase, 1, 1, 1, phase_dose_dev, 0u, false, true, dose4d_dev,
+                           stats);
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_accumulator_ptrs(pbs4d_ctx* ctx, int32_t src_phase, int64_t** e_dev, int64_t** m_dev) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (src_phase < 0 || src_phase >= ctx->n_phases || !e_dev || !m_dev)
+        return fail(ctx, PBS4D_ERR_ARG, "accumulator_ptrs: bad argument");
+    if (!ctx->have_acc[src_phase]) return fail(ctx, PBS4D_ERR_ORDER, "accumulator_ptrs: phase has no accumulators");
+    *e_dev = ctx->accE[src_phase]->as<int64_t>(); *m_dev = ctx->accM[src_phase]->as<int64_t>();
+    return PBS4D_OK;
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (src_phase < 0 || src_phase >= ctx->n_phases || !e_dev || !m_dev)
@@ -569,6 +731,70 @@ extern "C" int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t
     CU(cudaStreamSynchronize(ctx->stream));
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
+
+// ------------------------------------------------------------------------------------------------------------------
+// uncertainty trials: sampled delivery -> per-phase MC -> accumulation, per trial, context re-used
+// ------------------------------------------------------------------------------------------------------------------
+extern "C" int pbs4d_simulate_delivery_trial(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, int32_t trial,
+                                             const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
+                                             uint64_t total_histories, pbs4d_phase_lists* out, int64_t* n_fills) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!spec || !prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery_trial: null argument");
+    if (ctx->fields.empty()) return fail(ctx, PBS4D_ERR_ORDER, "simulate_delivery_trial: call set_plan_spots first");
+    const pbs4d_delivery_ext none{};
+    const pbs4d_delivery_ext& central = ext ? *ext : none;
+    const int32_t nf = (int32_t)ctx->fields.size();
+    std::vector<int32_t> start(nf);
+    std::vector<int64_t> cycles(std::max(spec->n_cycles, 1)), resets(std::max(central.n_layer_switch, 1));
+    pbs4d_delivery_params p{}; pbs4d_delivery_ext x{};
+    const int rc = sample_trial_host(*spec, trial, nf, *prm, central, start.data(), cycles.data(), resets.data(), p, x);
+    if (rc != PBS4D_OK) return fail(ctx, rc, "simulate_delivery_trial: bad trial specification");
+    for (int32_t f = 0; f < nf; ++f) ctx->fields[f].start_phase = start[f];
+    return pbs4d_simulate_delivery_ext(ctx, &p, &x, total_histories, out, n_fills);
+}
+catch (...) { return on_exception(ctx); }
+
+extern "C" int pbs4d_run_trials(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, int32_t first, int32_t count,
+                                const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
+                                uint64_t total_histories, uint64_t seed, int32_t ref_phase, int32_t nsx, int32_t nsy,
+                                int32_t nsz, float* const* dose4d_dev, pbs4d_trial_result* results) try
+{
+    if (!ctx) return PBS4D_ERR_ARG;
+    if (!spec || !prm || !dose4d_dev || first < 0 || count < 1 || first + count > spec->n_trials)
+        return fail(ctx, PBS4D_ERR_ARG, "run_trials: bad argument");
+    if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "run_trials: no densities (set_ct_phases)");
+    if (ref_phase < 0 || ref_phase >= ctx->n_phases) return fail(ctx, PBS4D_ERR_ARG, "run_trials: bad reference phase");
+    for (int32_t t = 0; t < count; ++t) {
+        if (!dose4d_dev[t]) return fail(ctx, PBS4D_ERR_ARG, "run_trials: null output buffer");
+        int64_t fills = 0;
+        int rc = pbs4d_simulate_delivery_trial(ctx, spec, first + t, prm, ext, total_histories, nullptr, &fills);
+        if (rc != PBS4D_OK) return rc;
+        std::vector<int32_t> todo;
+        for (int p = 0; p < ctx->n_phases && p < ctx->deliv_phases; ++p)
+            if (ctx->launches[p].n_hist > 0 || p == ref_phase) todo.push_back(p);
+        std::vector<pbs4d_mc_stats> st(todo.size());
+        float tr_ms = 0.0f;
+        std::fill(ctx->have_dose.begin(), ctx->have_dose.end(), false);     // doses of the previous trial are stale
+        rc = pbs4d_mc_dose_phases(ctx, (int32_t)todo.size(), todo.data(), seed + (uint64_t)(first + t), 0.0, st.data(),
+                                  &tr_ms);
+        if (rc != PBS4D_OK) return rc;
+        pbs4d_acc_stats as{};
+        rc = pbs4d_accumulate_subvoxel(ctx, ref_phase, nsx, nsy, nsz, nullptr, dose4d_dev[t], &as);
+        if (rc != PBS4D_OK) return rc;
+        if (results) {
+            pbs4d_trial_result& r = results[t];
+            r.histories = 0; for (const auto& s : st) r.histories += s.histories;
+            r.delivery_ns = 0; for (int64_t v : ctx->field_time) r.delivery_ns = std::max(r.delivery_ns, v);
+            r.fills = fills; r.phases_run = 0; r.pad = 0;
+            for (int p = 0; p < ctx->deliv_phases; ++p) r.phases_run += ctx->launches[p].n_hist > 0 ? 1 : 0;
+            r.transport_ms = tr_ms; r.accumulate_ms = as.push_ms + as.finalize_ms;
+        }
+    }
+    return PBS4D_OK;
+}
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // whole path with host buffers (end-to-end entry used by bench.py's e2e leg)
@@ -579,70 +805,91 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
                                    int32_t n_fields, const pbs4d_field* fields, int64_t n_spots, const pbs4d_spot* spots,
                                    const pbs4d_delivery_params* prm, uint64_t total_histories, uint64_t seed,
                                    int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
-                                   double* seconds)
+                                   uint64_t* h2d_bytes, double* seconds) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_host || !prm || !dose4d_host || ref_phase < 0 ||
-        ref_phase >= n_phases || prm->n_phases != n_phases || (disp_host && !grid_ok(dvf_grid)))
+        ref_phase >= n_phases || prm->n_phases != n_phases || (disp_host && !grid_ok(dvf_grid)) ||
+        (dose_grid && !grid_ok(dose_grid)) || n_pts < 2 || n_pts > 64 || !hu_pts || !rho_pts)
         return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: bad argument");
+    for (int i = 0; i < n_pts; ++i)
+        if (!(rho_pts[i] > 0.0f) || (i && !(hu_pts[i] > hu_pts[i - 1])))
+            return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: table must ascend in HU with positive densities");
+    for (int p = 0; p < n_phases; ++p)
+        if (!hu_host[p]) return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: null CT phase");
     using clk = std::chrono::steady_clock;
     auto sec = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
     CU(cudaSetDevice(ctx->device));
     const auto t0 = clk::now();
 
-    // H2D: CT phases -> densities, DVFs
+    // a2 + a3 first (host only, ~ms): the sub-plans say which breathing phases receive beam, and only those phases
+    // (plus the reference phase) need a density grid, a transport launch and -- as push sources -- a DVF.  With gating
+    // most phases of a 4DCT are idle (config 5: 4 of 10 active); their CT and DVF are not uploaded at all.
+    int rc = pbs4d_set_plan_spots(ctx, n_fields, fields, n_spots, spots);
+    if (rc != PBS4D_OK) return rc;
+    rc = pbs4d_simulate_delivery(ctx, prm, total_histories, nullptr);
+    if (rc != PBS4D_OK) return rc;
+    std::vector<int32_t> active;
+    for (int p = 0; p < n_phases; ++p)
+        if (ctx->launches[p].n_hist > 0 || p == ref_phase) active.push_back(p);
+    const auto t1 = clk::now();
+
+    // H2D: CT of the active phases -> densities (a1)
+    uint64_t bytes = 0;
+    const pbs4d_grid& g = dose_grid ? *dose_grid : *ct;
+    reset_phase_state(ctx, n_phases, g);
     const size_t ct_vox = (size_t)ct->nx * ct->ny * ct->nz;
     DevBuf& hu_dev = ctx->host_hu;
-    CU(hu_dev.ensure((size_t)n_phases * ct_vox * sizeof(int16_t)));
-    std::vector<const int16_t*> hu_ptrs(n_phases);
-    for (int p = 0; p < n_phases; ++p) {
-        if (!hu_host[p]) return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: null CT phase");
-        hu_ptrs[p] = hu_dev.as<int16_t>() + (size_t)p * ct_vox;
-        CU(cudaMemcpyAsync((void*)hu_ptrs[p], hu_host[p], ct_vox * sizeof(int16_t), cudaMemcpyHostToDevice, ctx->stream));
-    }
-    int rc = pbs4d_set_ct_phases(ctx, n_phases, ct, hu_ptrs.data(), dose_grid, n_pts, hu_pts, rho_pts);
-    if (rc != PBS4D_OK) return rc;
-    // DVFs are not needed before the accumulation: their upload (the bulk of the host->device bytes) and re-layout
-    // run on a copy stream underneath the delivery simulation and the transport kernels
-    struct CopyGuard {                                   // an early error return must not leave copies from the
-        cudaStream_t st = nullptr; cudaEvent_t ev = nullptr;   // caller's host buffers in flight
-        ~CopyGuard() { if (ev) { cudaStreamSynchronize(st); cudaEventDestroy(ev); } }
+    CU(hu_dev.ensure(active.size() * ct_vox * sizeof(int16_t)));
+    CU(ctx->table.ensure(2 * n_pts * sizeof(float)));
+    // an early error return must not leave copies from the caller's host buffers in flight: armed before the first copy
+    struct CopyGuard {
+        cudaStream_t st[2] = { nullptr, nullptr }; cudaEvent_t ev = nullptr; bool armed = false;
+        ~CopyGuard() { if (armed) { cudaStreamSynchronize(st[0]); cudaStreamSynchronize(st[1]); } if (ev) cudaEventDestroy(ev); }
     } guard;
+    if (disp_host && !ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    guard.st[0] = ctx->stream; guard.st[1] = ctx->copy_stream; guard.armed = true;
+    CU(cudaMemcpyAsync(ctx->table.p, hu_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->table.as<float>() + n_pts, rho_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    for (size_t a = 0; a < active.size(); ++a) {
+        const int p = active[a];
+        int16_t* dst = hu_dev.as<int16_t>() + a * ct_vox;
+        CU(cudaMemcpyAsync(dst, hu_host[p], ct_vox * sizeof(int16_t), cudaMemcpyHostToDevice, ctx->stream));
+        bytes += ct_vox * sizeof(int16_t);
+        CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
+        launch_hu_to_density(*ct, dst, dose_grid, n_pts, ctx->table.as<float>(), ctx->table.as<float>() + n_pts,
+                             ctx->rho[p]->as<float>(), ctx->stream);
+        ctx->rho_valid[p] = true;
+    }
+    CU(cudaGetLastError());
+    ctx->have_density = true;
+    // DVFs are not needed before the accumulation: their upload (the bulk of the host->device bytes) and re-layout
+    // run on a copy stream underneath the transport kernels
     cudaEvent_t& dvf_ready = guard.ev;
     if (disp_host) {
-        if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         const size_t dvf_vox = (size_t)dvf_grid->nx * dvf_grid->ny * dvf_grid->nz;
         DevBuf& tmp = ctx->host_dvf;
         CU(tmp.ensure(3 * dvf_vox * sizeof(float)));
-        for (int p = 0; p < n_phases; ++p) {
+        for (int p : active) {
             if (p == ref_phase || !disp_host[p]) continue;
             auto& d = ctx->dvf[p];
             if (!d.disp) d.disp.reset(new DevBuf);
             CU(d.disp->ensure(4 * dvf_vox * sizeof(float)));
             CU(cudaMemcpyAsync(tmp.p, disp_host[p], 3 * dvf_vox * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
+            bytes += 3 * dvf_vox * sizeof(float);
             launch_dvf_interleave(*dvf_grid, tmp.as<float>(), d.disp->as<float>(), ctx->copy_stream);
             d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
         }
         CU(cudaGetLastError());
-        guard.st = ctx->copy_stream;
         CU(cudaEventCreateWithFlags(&dvf_ready, cudaEventDisableTiming));
         CU(cudaEventRecord(dvf_ready, ctx->copy_stream));
     }
-    const auto t1 = clk::now();
-
-    rc = pbs4d_set_plan_spots(ctx, n_fields, fields, n_spots, spots);
-    if (rc != PBS4D_OK) return rc;
-    rc = pbs4d_simulate_delivery(ctx, prm, total_histories, nullptr);
-    if (rc != PBS4D_OK) return rc;
     const auto t2 = clk::now();
 
     uint64_t run = 0;
     {
-        std::vector<int32_t> todo;
-        for (int p = 0; p < n_phases; ++p)
-            if (ctx->launches[p].n_hist > 0 || p == ref_phase) todo.push_back(p);
-        std::vector<pbs4d_mc_stats> st(todo.size());
-        rc = pbs4d_mc_dose_phases(ctx, (int32_t)todo.size(), todo.data(), seed, 0.0, st.data(), nullptr);
+        std::vector<pbs4d_mc_stats> st(active.size());
+        rc = pbs4d_mc_dose_phases(ctx, (int32_t)active.size(), active.data(), seed, 0.0, st.data(), nullptr);
         if (rc != PBS4D_OK) return rc;
         for (const auto& x : st) run += x.histories;
     }
@@ -657,14 +904,16 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     CU(cudaStreamSynchronize(ctx->stream));
     const auto t4 = clk::now();
     if (histories_run) *histories_run = run;
+    if (h2d_bytes) *h2d_bytes = bytes + (uint64_t)n_spots * sizeof(pbs4d_spot) + (uint64_t)n_fields * sizeof(pbs4d_field);
     if (seconds) { seconds[0] = sec(t0, t1); seconds[1] = sec(t1, t2); seconds[2] = sec(t2, t3); seconds[3] = sec(t3, t4); }
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // in-run roofline probes
 // ------------------------------------------------------------------------------------------------------------------
-extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value)
+extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!value || kind < PBS4D_PROBE_FP32_ISSUE || kind > PBS4D_PROBE_HBM_COPY)
@@ -679,12 +928,13 @@ extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value)
     }
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // dose-interpolation accumulation (DIM, Eq. 3): pull every source phase with a T^{R->S} field
 // ------------------------------------------------------------------------------------------------------------------
 extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
-                                    const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats)
+                                    const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_dim: no grid (set_ct_phases/set_density_phases)");
@@ -733,12 +983,13 @@ extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t n
     }
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }
 
 // ------------------------------------------------------------------------------------------------------------------
 // DVF construction from DICOM minimal grid information
 // ------------------------------------------------------------------------------------------------------------------
 extern "C" int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, const float* delta_dev, float* rf_dev,
-                               float* disp_dev, pbs4d_grid* grid_out)
+                               float* disp_dev, pbs4d_grid* grid_out) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
     if (!info || !delta_dev || (!rf_dev && !disp_dev) || info->nx < 1 || info->ny < 1 || info->nz < 1 ||
@@ -761,3 +1012,4 @@ extern "C" int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, cons
     CU(cudaStreamSynchronize(ctx->stream));
     return PBS4D_OK;
 }
+catch (...) { return on_exception(ctx); }

@@ -327,7 +327,7 @@ extern "C" int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field*
                                             const pbs4d_spot* spots, const pbs4d_delivery_params* prm,
                                             uint64_t total_histories, pbs4d_segment* segs_out, int64_t max_segs,
                                             int64_t* n_segs_out, int64_t* field_time_ns, int64_t* dropped_protons,
-                                            int32_t* fixed_shift)
+                                            int32_t* fixed_shift) try
 {
     if (n_fields < 1 || !fields || n_spots < 1 || !spots || !prm || !n_segs_out) return PBS4D_ERR_ARG;
     std::vector<pbs4d_field> f(fields, fields + n_fields);
@@ -346,13 +346,14 @@ extern "C" int pbs4d_simulate_delivery_host(int32_t n_fields, const pbs4d_field*
     if (fixed_shift) *fixed_shift = pbs4d::fixed_shift_for(segs, s);
     return PBS4D_OK;
 }
+catch (...) { return PBS4D_ERR_NOMEM; }     // std::bad_alloc: nothing throws across the C boundary
 
 extern "C" int pbs4d_simulate_delivery_ext_host(int32_t n_fields, const pbs4d_field* fields, int64_t n_spots,
                                                 const pbs4d_spot* spots, const pbs4d_delivery_params* prm,
                                                 const pbs4d_delivery_ext* ext, uint64_t total_histories,
                                                 pbs4d_segment* segs_out, int64_t max_segs, int64_t* n_segs_out,
                                                 int64_t* field_time_ns, int64_t* dropped_protons, int32_t* fixed_shift,
-                                                int64_t* n_fills)
+                                                int64_t* n_fills) try
 {
     if (n_fields < 1 || !fields || n_spots < 1 || !spots || !prm || !ext || !n_segs_out) return PBS4D_ERR_ARG;
     std::vector<pbs4d_field> f(fields, fields + n_fields);
@@ -372,3 +373,4 @@ extern "C" int pbs4d_simulate_delivery_ext_host(int32_t n_fields, const pbs4d_fi
     if (n_fills) *n_fills = fills;
     return PBS4D_OK;
 }
+catch (...) { return PBS4D_ERR_NOMEM; }     // std::bad_alloc: nothing throws across the C boundary

@@ -74,16 +74,31 @@ __global__ void hu_to_density_resample(pbs4d_grid ct, pbs4d_grid dg, const int16
     out[((size_t)z * dg.ny + y) * dg.nx + x] = (float)(wsum > 0.0 ? acc / wsum : (double)rp[0]);
 }
 
-// a7 / T12: D = Q 2^-k 1.602176634e-10 / (rho V_cm3)  [Gy]; optionally per proton
+// a7 / T12: D = Q 2^-k 1.602176634e-10 / (rho V_cm3)  [Gy]; optionally per proton.  A voxel without mass (never the
+// case for densities accepted by set_ct_phases / set_density_phases) gets dose 0 instead of 0/0.
 __global__ void finalize_dose_kernel(long long nvox, const float* __restrict__ rho, const long long* __restrict__ Q,
                                      double inv_scale, double vol_cm3, double per_protons, float* __restrict__ dose)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride) {
-        double D = (double)Q[i] * inv_scale * 1.602176634e-10 / ((double)rho[i] * vol_cm3);
+        const double mass = (double)rho[i] * vol_cm3;
+        double D = (double)Q[i] * inv_scale * 1.602176634e-10 / mass;
         if (per_protons > 0.0) D /= per_protons;
-        dose[i] = (float)D;
+        dose[i] = mass > 0.0 ? (float)D : 0.0f;
     }
+}
+
+// densities handed in directly (set_density_phases) must be finite and inside [kRhoMin, kRhoMax]: rho = 0 would give
+// 0/0 in the dose, rho = Inf a zero step limit (a history that never advances)
+__global__ void validate_density_kernel(size_t n, const float* __restrict__ rho, int* __restrict__ bad)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    bool any = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const float r = rho[i];
+        any |= !(r >= 1.0e-6f && r <= 100.0f);               // also true for NaN
+    }
+    if (__any_sync(0xffffffffu, any) && (threadIdx.x & 31) == 0) atomicOr(bad, 1);
 }
 
 
@@ -152,15 +167,27 @@ void launch_dvf_build(const pbs4d_dicom_dvf& g, const float* delta_dev, float* r
     dvf_build_kernel<<<grid, 256, 0, st>>>(P);
 }
 
-namespace {
-}  // namespace
+int sm_count_of_current_device(void)
+{
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    return n;
+}
+
+int launch_validate_density(const float* rho, size_t n, int* flag_dev, cudaStream_t st)
+{
+    const int blocks = (int)min((long long)((n + 255) / 256), (long long)sm_count_of_current_device() * 16);
+    validate_density_kernel<<<blocks, 256, 0, st>>>(n, rho, flag_dev);
+    return 0;
+}
 
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
                           const float* hp, const float* rp, float* rho_out, cudaStream_t st)
 {
     if (!dose_grid) {
         const long long nvox = (long long)ct.nx * ct.ny * ct.nz;
-        const int blocks = (int)min((nvox + 255) / 256, (long long)148 * 16);
+        const int blocks = (int)min((nvox + 255) / 256, (long long)sm_count_of_current_device() * 16);
         hu_to_density_same_grid<<<blocks, 256, 0, st>>>(nvox, hu, n_pts, hp, rp, rho_out);
     } else {
         dim3 b(32, 8, 1), g((dose_grid->nx + 31) / 32, (dose_grid->ny + 7) / 8, dose_grid->nz);
@@ -173,7 +200,7 @@ void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long
 {
     const long long nvox = (long long)g.nx * g.ny * g.nz;
     const double vol_cm3 = (double)g.hx * (double)g.hy * (double)g.hz * 1.0e-3;
-    const int blocks = (int)min((nvox + 255) / 256, (long long)148 * 16);
+    const int blocks = (int)min((nvox + 255) / 256, (long long)sm_count_of_current_device() * 16);
     finalize_dose_kernel<<<blocks, 256, 0, st>>>(nvox, rho, Q, ldexp(1.0, -fixed_shift), vol_cm3, per_protons, dose);
 }
 

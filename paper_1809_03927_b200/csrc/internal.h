@@ -24,6 +24,9 @@ int simulate_delivery_ext_host(const std::vector<pbs4d_field>& fields, const std
                                uint64_t total_histories, std::vector<pbs4d_segment>& segments,
                                std::vector<int64_t>& field_time_ns, int64_t& dropped_protons, int64_t& n_fills,
                                std::string& err);
+int sample_trial_host(const pbs4d_trial_spec& spec, int32_t trial, int32_t n_fields, const pbs4d_delivery_params& prm,
+                      const pbs4d_delivery_ext& ext, int32_t* start_phase, int64_t* cycle_period_ns,
+                      int64_t* layer_switch_ns, pbs4d_delivery_params& prm_out, pbs4d_delivery_ext& ext_out);
 int32_t fixed_shift_for(const std::vector<pbs4d_segment>& segments, const std::vector<pbs4d_spot>& spots);
 
 // ---- device-side segment record (transport.cu): everything a history needs from its (field, spot) ----
@@ -45,10 +48,19 @@ struct TransportCounters {       // device tallies of one launch (zeroed before 
 };
 
 // Launchers (all asynchronous on `st`).
+// hist_begin / n_hist: window of the phase's local history range this launch transports (sharding); phys_tab_dev: the
+// context's copy of the physics table (physics_tables.h), physics_table_bytes() bytes.
 void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, const long long* seg_begin,
-                      int32_t n_segs, int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q,
-                      TransportCounters* counters, int sm_count, cudaStream_t st);
+                      int32_t n_segs, int64_t hist_begin, int64_t n_hist, uint64_t seed, uint32_t flags,
+                      const void* phys_tab_dev, long long* Q, TransportCounters* counters, int sm_count, cudaStream_t st);
 const void* transport_kernel_symbol();
+size_t physics_table_bytes(void);
+void build_physics_table_host(void* nodes /* physics_table_bytes() */);
+#ifdef __CUDACC__
+cudaError_t configure_transport(void);            // per-device kernel attributes (current device)
+cudaError_t configure_accumulate(void);
+int launch_validate_density(const float* rho, size_t n, int* flag_dev, cudaStream_t st);
+#endif
 
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
                           const float* hu_pts_dev, const float* rho_pts_dev, float* rho_out, cudaStream_t st);
@@ -62,6 +74,7 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
                       const float* disp4, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
                       long long* E, long long* M, AccCounters* counters, cudaStream_t st);
 // out = (first ? dose_ref : out_acc) ... see accumulate.cu: ratio-and-add over all pushed phases, then mask.
+int sm_count_of_current_device(void);
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_dev,
                           const long long* const* M_dev, const pbs4d_grid* dvf_grids_dev,
                           unsigned char* flags_dev /*[nx+ny+nz] scratch*/, float* out, cudaStream_t st);

@@ -64,4 +64,7 @@ void build_physics_table(TabNode* nodes)
     }
 }
 
+// untyped entry for api.cu (which does not see the node layout): fills physics_table_bytes() bytes
+void build_physics_table_host(void* nodes) { build_physics_table(static_cast<TabNode*>(nodes)); }
+
 }  // namespace pbs4d

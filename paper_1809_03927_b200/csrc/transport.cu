@@ -49,7 +49,7 @@ struct Params {
     const long long* __restrict__ seg_begin;  // [n_segs] local index of each segment's first history (ascending)
     const float4* __restrict__ tab;           // kTabNodes physics nodes
     int32_t n_segs;
-    long long n_hist;
+    long long hist_begin, n_hist;             // this launch transports local histories hist_begin .. hist_begin + n_hist - 1
     uint32_t flags;
     uint32_t k0[10], k1[10];                  // Philox round keys
     unsigned long long* Q;
@@ -253,7 +253,7 @@ transport_kernel(const __grid_constant__ Params P)
                 if (j < P.n_hist) {
                     Lane T;
                     long long qi = 0, qe = 0;
-                    const bool ok = start_history(P, j, T, qi, qe);
+                    const bool ok = start_history(P, P.hist_begin + j, T, qi, qe);
                     atomicAdd((unsigned long long*)&s_tally[0], 1ull);
                     atomicAdd((unsigned long long*)&s_tally[2], (unsigned long long)qi);
                     if (qe) atomicAdd((unsigned long long*)&s_tally[4], (unsigned long long)qe);
@@ -441,31 +441,25 @@ transport_kernel(const __grid_constant__ Params P)
 
 const void* transport_kernel_symbol() { return (const void*)transport_kernel; }
 
-static float4* g_tab_dev[16] = { nullptr };   // one table per device, built on first use
+cudaError_t configure_transport(void)
+{
+    // 22.5 KB table + 10 KB history pools per CTA: ask for a shared-memory carve-out that keeps 4 CTAs resident.
+    // A per-device attribute: pbs4d_create calls this once for every context (any device).
+    return cudaFuncSetAttribute(transport_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+}
+
+size_t physics_table_bytes(void) { return sizeof(TabNode) * kTabNodes; }
 
 void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* segs, const long long* seg_begin,
-                      int32_t n_segs, int64_t n_hist, uint64_t seed, uint32_t flags, long long* Q,
-                      TransportCounters* counters, int sm_count, cudaStream_t st)
+                      int32_t n_segs, int64_t hist_begin, int64_t n_hist, uint64_t seed, uint32_t flags,
+                      const void* phys_tab_dev, long long* Q, TransportCounters* counters, int sm_count, cudaStream_t st)
 {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dev >= 0 && dev < 16 && !g_tab_dev[dev]) {
-        static TabNode host_tab[kTabNodes];
-        build_physics_table(host_tab);
-        cudaMalloc(&g_tab_dev[dev], sizeof(host_tab));
-        cudaMemcpy(g_tab_dev[dev], host_tab, sizeof(host_tab), cudaMemcpyHostToDevice);
-    }
     Params P;
-    P.g = g; P.rho = rho; P.segs = segs; P.seg_begin = seg_begin; P.tab = g_tab_dev[dev];
-    P.n_segs = n_segs; P.n_hist = n_hist; P.flags = flags;
+    P.g = g; P.rho = rho; P.segs = segs; P.seg_begin = seg_begin; P.tab = static_cast<const float4*>(phys_tab_dev);
+    P.n_segs = n_segs; P.hist_begin = hist_begin; P.n_hist = n_hist; P.flags = flags;
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
     P.Q = (unsigned long long*)Q; P.counters = counters;
-    static bool configured = false;
-    if (!configured) {        // 22.5 KB table per CTA: ask for a shared-memory carve-out that keeps all CTAs resident
-        cudaFuncSetAttribute(transport_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
-        configured = true;
-    }
     int per_sm = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, transport_kernel, kThreads, 0);
     if (per_sm < 1) per_sm = 1;

@@ -36,10 +36,14 @@ def test_run_plan_host_equals_stepwise_path(name, kw):
     g = cfg["ct_grid"] if cfg["dose_grid"] is None else cfg["dose_grid"]
     out = np.full((int(g["nz"][0]), int(g["ny"][0]), int(g["nx"][0])), -1.0, np.float32)
     for rep in range(2):                                     # second call reuses the staging buffers
-        run, secs = ctx2.run_plan_host(cfg["ct_grid"], [cfg["hu"][p] for p in range(P)], cfg["dose_grid"], cfg["dvf_grid"],
+        run, secs, h2d = ctx2.run_plan_host(cfg["ct_grid"], [cfg["hu"][p] for p in range(P)], cfg["dose_grid"], cfg["dvf_grid"],
                                        cfg["dvf"], cfg["ref_phase"], cfg["fields"], cfg["spots"], cfg["deliv"],
                                        cfg["histories"], cfg["seed"], cfg["subvox"], out)
         assert run == n == cfg["histories"] and len(secs) == 4 and all(s >= 0 for s in secs)
         assert out.view(np.uint32).tobytes() == want.view(np.uint32).tobytes()
         assert want.max() > 0
+        # only the phases that receive beam (plus the reference phase) are uploaded, CT and DVF
+        expect = sum(cfg["hu"][p].nbytes for p in phases) + cfg["spots"].nbytes + cfg["fields"].nbytes + \
+            sum(cfg["dvf"][p].nbytes for p in phases if p != cfg["ref_phase"] and cfg["dvf"][p] is not None)
+        assert h2d == expect
     ctx2.close()
