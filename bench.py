@@ -170,6 +170,52 @@ def share_accumulators(pairs, owners, world):
             dist.broadcast(t, src=owners[p])
 
 
+def run_pass(ctx, cfg, hu_dev, dvf_dev, rank, world, sum_grids=sum_energy_grids, share=share_accumulators):
+    """One pass of the whole path with inputs resident in HBM.  world > 1: this rank's shard --
+    its slice of every phase's history range, then the integer all-reduce of the energy grids (`sum_grids`), a7 again,
+    the push of the source phases this rank owns, the exchange of the int64 sums (`share`) and a9.
+    Returns (histories transported here, 4D dose tensor, stats dict)."""
+    P = cfg["hu"].shape[0]
+    shape = ctx_shape(cfg)
+    nvox = int(np.prod(shape)); n_sub = int(np.prod(cfg["subvox"]))
+    ctx.set_ct_phases(cfg["ct_grid"], [hu_dev[p] for p in range(P)], cfg["dose_grid"])
+    for p in range(P):
+        if dvf_dev[p] is not None:
+            ctx.set_dvf(p, cfg["ref_phase"], cfg["dvf_grid"], dvf_dev[p])
+    ctx.set_plan_spots(cfg["fields"], cfg["spots"])
+    deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
+    phases = sorted(set(int(x) for x in deliv["segments"]["phase"]) | {cfg["ref_phase"]})
+    ctx.set_shard(rank, world)
+    sts, t_ms = ctx.mc_dose_phases(phases, cfg["seed"])              # all phases, concurrent launches; t_ms = fork..join
+    n_hist = sum(st["histories"] for st in sts)
+    n_dvf = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])          # fields re-laid out
+    src = [p for p in phases if p != cfg["ref_phase"] and dvf_dev[p] is not None]
+    extra = 0
+    if world == 1:
+        out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
+    else:
+        sum_grids([ctx.phase_energy_view(p) for p in phases], world)                               # the exchange step
+        for p in phases:
+            ctx.finalize_phase_dose(p)
+        owners = source_owners(src, world)
+        ast = ctx.accumulate_push(cfg["ref_phase"], cfg["subvox"], owner_mask(owners, rank))
+        share({p: ctx.accumulator_views(p) for p in src}, owners, world)
+        out, fst = ctx.accumulate_finalize(cfg["ref_phase"])
+        ast["finalize_ms"] = fst["finalize_ms"]
+        extra = len(phases)                                                                        # second a7 launches
+    ctx.set_shard(0, 1)
+    n_src = int(ast["subvoxels"]) // (nvox * n_sub)                                               # phases pushed here
+    # kernels launched: HU->density per phase, DVF interleave per source phase, transport per phase with histories
+    # here, dose finalize per phase run (twice when sharded), push per source phase pushed here, coverage flags +
+    # accumulation finalize
+    n_tr = sum(1 for st in sts if st["histories"] > 0)
+    stats = dict(histories=n_hist, mc_steps=sum(st["steps"] for st in sts), reds=sum(st["scoring_atomics"] for st in sts),
+                 transport_ms=t_ms, push_ms=ast["push_ms"], finalize_ms=ast["finalize_ms"], phases=len(phases),
+                 n_src=n_src, subvoxels=ast["subvoxels"], launches=P + n_dvf + n_tr + len(phases) + extra + n_src + 2,
+                 active=phases, src=src)
+    return n_hist, out, stats
+
+
 def reduce_over_ranks(ms, e2e_s, hist, hist_e2e, world, device):
     """Times -> MAX over ranks, histories -> SUM over ranks (whole-job throughput = all histories / slowest rank's
     time)."""
@@ -248,43 +294,9 @@ def main():
     stats = {}
 
     def step_device():
-        """one pass of the whole path, inputs resident in HBM"""
-        ctx.set_ct_phases(cfg["ct_grid"], [hu_dev[p] for p in range(P)], cfg["dose_grid"])
-        for p in range(P):
-            if dvf_dev[p] is not None:
-                ctx.set_dvf(p, cfg["ref_phase"], cfg["dvf_grid"], dvf_dev[p])
-        ctx.set_plan_spots(cfg["fields"], cfg["spots"])
-        deliv = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
-        phases = sorted(set(int(x) for x in deliv["segments"]["phase"]) | {cfg["ref_phase"]})
-        ctx.set_shard(rank, world)
-        sts, t_ms = ctx.mc_dose_phases(phases, cfg["seed"])          # all phases, concurrent launches; t_ms = fork..join
-        n_hist = sum(st["histories"] for st in sts); n_steps = sum(st["steps"] for st in sts)
-        n_red = sum(st["scoring_atomics"] for st in sts)
-        n_dvf = sum(1 for p in range(P) if dvf_dev[p] is not None and p != cfg["ref_phase"])      # fields re-laid out
-        src = [p for p in phases if p != cfg["ref_phase"] and dvf_dev[p] is not None]
-        extra = 0
-        if world == 1:
-            out, ast = ctx.accumulate_subvoxel(cfg["ref_phase"], cfg["subvox"])
-            n_src = int(ast["subvoxels"]) // (nvox * n_sub)                                       # phases really pushed
-        else:
-            sum_energy_grids([ctx.phase_energy_view(p) for p in phases], world)                   # the exchange step
-            for p in phases:
-                ctx.finalize_phase_dose(p)
-            owners = source_owners(src, world)
-            ast = ctx.accumulate_push(cfg["ref_phase"], cfg["subvox"], owner_mask(owners, rank))
-            share_accumulators({p: ctx.accumulator_views(p) for p in src}, owners, world)
-            out, fst = ctx.accumulate_finalize(cfg["ref_phase"])
-            ast["finalize_ms"] = fst["finalize_ms"]
-            n_src = int(ast["subvoxels"]) // (nvox * n_sub)
-            extra = len(phases)                                                                    # second a7 launches
-        # kernels launched: HU->density per phase, DVF interleave per source phase, transport + dose finalize per
-        # phase run, push per source phase pushed here, coverage flags + accumulation finalize
-        n_tr = sum(1 for st in sts if st["histories"] > 0)
-        stats.update(histories=n_hist, mc_steps=n_steps, reds=n_red, transport_ms=t_ms, push_ms=ast["push_ms"],
-                     finalize_ms=ast["finalize_ms"], phases=len(phases), n_src=n_src, subvoxels=ast["subvoxels"],
-                     launches=P + n_dvf + n_tr + len(phases) + extra + n_src + 2, checksum=float(out.sum()),
-                     active=phases, src=src)
-        return n_hist, out
+        n, out, st = run_pass(ctx, cfg, hu_dev, dvf_dev, rank, world)
+        stats.update(st)
+        return n, out
 
     out_host = np.zeros(ctx_shape(cfg), np.float32)
     torch.cuda.cudart().cudaHostRegister(out_host.ctypes.data, out_host.nbytes, 0)

@@ -548,8 +548,8 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     P.E = (unsigned long long*)E; P.M = (unsigned long long*)M; P.counters = counters;
     // z-chunk per thread: the x/y-lerps are evaluated once per z-node of a column, and the first node of a column is
     // extra, so longer columns amortise it (and the CTA prologue); measured on config 4 (chunk 1 -> this choice):
-    // n = 4 5.09 -> 4.19 ms, n = 8 29.9 -> 27.8 ms, (2,2,5) 1.69 -> 1.45 ms per 9 phases of 128^3
-    P.chunk_z = nsz <= 2 ? kChunkZMax : (nsz <= 4 ? 4 : 2);
+    // n = 4 5.09 -> 4.19 ms, n = 8 29.9 -> 27.4 ms, (2,2,5) 1.69 -> 1.34 ms per 9 phases of 128^3
+    P.chunk_z = nsz <= 2 ? kChunkZMax : 4;
     dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY,
                                  (src.nz + P.chunk_z - 1) / P.chunk_z);
     const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +

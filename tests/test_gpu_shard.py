@@ -121,3 +121,57 @@ def test_density_validation_rejects_zero_and_nonfinite(ctx):
         bad = good.clone(); bad[1, 2, 3] = bad_value
         with pytest.raises(RuntimeError, match="densities must be finite"):
             ctx.set_density_phases(g, [good, bad])
+
+
+def test_bench_pass_sharded_equals_single(ctx):
+    """bench.py's N > 1 pass (run_pass), driven for world = 2 on one device: the two ranks run one after the other and
+    the collectives are replaced by stand-ins that move the same integers (sum of the energy grids, owner's sums to
+    everyone).  The 4D dose of the sharded pass must equal the single-GPU pass bit for bit."""
+    import bench
+    cfg = synth.config5(div=8, n_hist=80_000)
+    P = cfg["hu"].shape[0]
+    hu_dev = torch.from_numpy(cfg["hu"]).cuda()
+    dvf_dev = [None if d is None else torch.from_numpy(d).cuda() for d in cfg["dvf"]]
+    n1, out1, st1 = bench.run_pass(ctx, cfg, hu_dev, dvf_dev, 0, 1)
+    out1 = out1.clone()
+    world = 2
+    # pass A: every rank transports its slice; keep its grids
+    grids = {}
+
+    def record(r):
+        def sum_grids(views, w):
+            grids[r] = [v.clone() for v in views]
+        return sum_grids
+
+    pushed = {}
+
+    def record_push(r):
+        def share(pairs, owners, w):
+            for p, (E, M) in pairs.items():
+                if owners[p] == r:
+                    pushed[p] = (E.clone(), M.clone())
+        return share
+
+    hist = 0
+    for r in range(world):
+        n, _, st = bench.run_pass(ctx, cfg, hu_dev, dvf_dev, r, world, sum_grids=record(r), share=lambda *a: None)
+        hist += n
+    assert hist == n1 == cfg["histories"]
+    total = [sum(grids[r][i] for r in range(world)) for i in range(len(grids[0]))]
+
+    # pass B: the same passes with the exchanges delivering what the collectives would
+    def all_reduce_stub(views, w):
+        for v, t in zip(views, total):
+            v.copy_(t)
+
+    for r in range(world):                                     # first collect every owner's sums (from summed grids)
+        bench.run_pass(ctx, cfg, hu_dev, dvf_dev, r, world, sum_grids=all_reduce_stub, share=record_push(r))
+
+    def broadcast_stub(pairs, owners, w):
+        for p, (E, M) in pairs.items():
+            E.copy_(pushed[p][0]); M.copy_(pushed[p][1])
+
+    for r in range(world):
+        n, out, st = bench.run_pass(ctx, cfg, hu_dev, dvf_dev, r, world, sum_grids=all_reduce_stub, share=broadcast_stub)
+        assert torch.equal(out.view(torch.int32), out1.view(torch.int32)), f"rank {r}"
+        assert st["launches"] > 0 and st["phases"] == st1["phases"]
