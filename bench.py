@@ -51,7 +51,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config5", choices=["config5", "config3", "config2"])
+    ap.add_argument("--workload", default="config5", choices=["config5", "config3", "config2", "config4"],
+                    help="config5 (default, the metric's config), config3, config2: the whole path; config4: the "
+                         "accumulation stress of BASELINE.json config 4 alone (push / DIM at n = 2, 4, 8 and (2,2,5))")
     ap.add_argument("--histories", type=int, default=0, help="override the config's history count (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -170,6 +172,70 @@ def share_accumulators(pairs, owners, world):
             dist.broadcast(t, src=owners[p])
 
 
+def run_accumulation_stress(args):
+    """--workload config4 (BASELINE.json:10): 10 phase doses of 128^3 at 2 mm, random smooth DVFs |u| <= 20 mm,
+    accumulated onto phase 0 at subvoxel edges 1.0 / 0.5 / 0.25 mm (n = 2, 4, 8) and at (2,2,5); EMTM push + finalize and
+    the DIM pull, each against BOTH rooflines (algorithmic HBM bytes, executed lane-instructions from profiles/).
+    One JSON line; launch order is fixed (per subdivision: warm-up + timed calls of 9 source phases each), which is what
+    the ncu captures under profiles/ index with -s."""
+    import torch
+    from paper_1809_03927_b200 import binding, build, synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the pbs4d path has no CPU fallback")
+    build.build()
+    c = synth.config4()
+    ctx = binding.Context(0)
+    P = len(c["doses"])
+    rho = torch.from_numpy(c["rhos"]).cuda(); dose = torch.from_numpy(c["doses"]).cuda()
+    ctx.set_density_phases(c["grid"], [rho[p] for p in range(P)])
+    disp = [None if d is None else torch.from_numpy(d).cuda() for d in c["disps"]]
+    for p in range(P):
+        if disp[p] is not None:
+            ctx.set_dvf(p, c["ref_phase"], c["dvf_grid"], disp[p])
+            ctx.set_dvf_pull(p, c["ref_phase"], c["dvf_grid"], disp[p])
+    doses = [dose[p] for p in range(P)]
+    n_src = sum(1 for d in disp if d is not None)
+    nvox = int(np.prod(c["doses"].shape[1:]))
+    peaks, peak_kind = measured_peaks()
+    prof = profile_metrics()
+    props = torch.cuda.get_device_properties(0)
+    issue_peak = props.multi_processor_count * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    warm, steps = max(args.warmup, 1) if args.warmup != 3 else 1, args.steps if args.steps != 3 else 2
+
+    def timed(fn, ns):
+        ms = fin = 0.0
+        for i in range(warm + steps):
+            _, st = fn(c["ref_phase"], ns, doses)
+            if i >= warm:
+                ms += st["push_ms"]; fin += st["finalize_ms"]
+        return ms / steps, fin / steps, st
+
+    out = {"metric": "subvoxels/s (accumulation stress)", "unit": "subvoxels/s", "n_gpus": 1, "steps": steps,
+           "warmup": warm, "higher_is_better": True, "dtype": "f32+i64", "data": "synthetic",
+           "config": {"workload": "config4", "grid": list(c["doses"].shape[1:]), "source_phases": n_src},
+           "peaks": {"hbm_GBps": peaks["hbm_gbs"], "issue_Tlaneops": issue_peak, "kind": peak_kind}, "push": {}, "dim": {}}
+    for ns in [(2, 2, 2), (4, 4, 4), (8, 8, 8), (2, 2, 5)]:
+        ms, fin, st = timed(ctx.accumulate_subvoxel, ns)
+        key = "x".join(map(str, ns))
+        ops = prof.get(("emtm_push_kernel", f"config4_{key}", "thread_inst_per_subvoxel"))
+        rate = st["subvoxels"] / (ms * 1e-3)
+        gbs = n_src * nvox * 36 / (ms * 1e-3) / 1e9
+        out["push"][key] = {"ms": ms, "subvoxels_per_s": rate, "hbm_GBps": gbs, "hbm_frac": gbs / peaks["hbm_gbs"],
+                            "lane_ops_per_subvoxel": ops, "issue_frac": None if not ops else rate * ops / 1e12 / issue_peak,
+                            "finalize_ms": fin, "finalize_GBps": nvox * (16 * n_src + 8) / (fin * 1e-3) / 1e9}
+    for ns in [(1, 1, 1), (2, 2, 2), (4, 4, 4), (8, 8, 8)]:
+        ms, fin, st = timed(ctx.accumulate_dim, ns)
+        key = "x".join(map(str, ns))
+        ops = prof.get(("dim_pull_kernel", f"config4_{key}", "thread_inst_per_subvoxel"))
+        rate = st["subvoxels"] / (ms * 1e-3)
+        gbs = n_src * nvox * 36 / (ms * 1e-3) / 1e9                 # DVF float4 + dose + double accumulator RMW per voxel
+        out["dim"][key] = {"ms": ms, "subvoxels_per_s": rate, "hbm_GBps": gbs, "hbm_frac": gbs / peaks["hbm_gbs"],
+                           "lane_ops_per_subvoxel": ops, "issue_frac": None if not ops else rate * ops / 1e12 / issue_peak}
+    out["value"] = out["push"]["2x2x2"]["subvoxels_per_s"]
+    print(json.dumps(out), flush=True)
+    ctx.close()
+
+
 def run_pass(ctx, cfg, hu_dev, dvf_dev, rank, world, sum_grids=sum_energy_grids, share=share_accumulators):
     """One pass of the whole path with inputs resident in HBM.  world > 1: this rank's shard --
     its slice of every phase's history range, then the integer all-reduce of the energy grids (`sum_grids`), a7 again,
@@ -234,6 +300,8 @@ def run_reference(args, rank, world):
     """--impl reference: the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
     if rank != 0:
         return
+    if args.workload == "config4":
+        raise SystemExit("--impl reference times the transport oracle; use --workload config5 | config3 | config2")
     cfg = make_workload(args.workload, 0, args.histories)
     budget = ORACLE_SAMPLE[args.workload] // 2
     rates, text, cores = [], "", 0
@@ -259,6 +327,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.workload == "config4":
+        if rank == 0:
+            run_accumulation_stress(args)
         return
 
     import torch

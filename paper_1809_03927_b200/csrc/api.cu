@@ -65,6 +65,8 @@ struct pbs4d_ctx {
     pbs4d_grid dose_grid{};
     std::vector<std::unique_ptr<DevBuf>> rho;            // [phase] fp32 on dose grid
     std::vector<bool> rho_valid;                         // [phase] density grid filled (run_plan_host fills active phases only)
+    std::vector<cudaEvent_t> rho_ready;                  // [phase] density grid complete on the copy stream (run_plan_host)
+    std::vector<bool> rho_pending;                       // [phase] the next transport launch must wait for rho_ready
     DevBuf table;                                        // hu_pts | rho_pts
 
     // DVFs (a2)
@@ -93,8 +95,11 @@ struct pbs4d_ctx {
     DevBuf phys_tab;                                     // per-energy physics table of the transport kernel (per context)
     int32_t shard_rank = 0, shard_world = 1;             // history sharding (pbs4d_set_shard)
     std::vector<std::unique_ptr<DevBuf>> seg_phase;      // [phase] launch table (DevSegment[] | seg_begin[])
+    std::vector<bool> seg_resident;                      // [phase] launch table of the current delivery is on the device
     std::vector<cudaStream_t> aux;                       // auxiliary streams for concurrent phase launches
-    cudaStream_t copy_stream = nullptr;                  // uploads that overlap compute (run_plan_host)
+    cudaStream_t copy_stream = nullptr;                  // uploads that overlap compute (run_plan_host): DMA only
+    cudaStream_t prep_stream = nullptr;                  // HU -> density and DVF re-layout kernels behind the uploads
+    std::vector<cudaEvent_t> upload_done;                // [2 * phase + {0: CT, 1: DVF}] copy finished on copy_stream
 
     // accumulation state (a8-a9)
     std::vector<std::unique_ptr<DevBuf>> accE, accM;     // [phase]
@@ -159,6 +164,7 @@ void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
     ctx->have_dose.assign(n_phases, false);
     ctx->have_acc.assign(n_phases, false);
     ctx->rho_valid.assign(n_phases, false);
+    ctx->rho_pending.assign(n_phases, false);
     ctx->have_density = false;
 }
 
@@ -200,7 +206,10 @@ void pbs4d_destroy(pbs4d_ctx* ctx) try
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (auto st : ctx->aux) if (st) cudaStreamDestroy(st);
+    for (auto e : ctx->rho_ready) if (e) cudaEventDestroy(e);
     if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    if (ctx->prep_stream) { cudaStreamSynchronize(ctx->prep_stream); cudaStreamDestroy(ctx->prep_stream); }
+    for (auto e : ctx->upload_done) if (e) cudaEventDestroy(e);
     delete ctx;
 }
 catch (...) {}
@@ -403,6 +412,7 @@ extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_
         L.n_hist += sg.n_hist;
     }
     ctx->have_delivery = true;
+    std::fill(ctx->seg_resident.begin(), ctx->seg_resident.end(), false);
     std::fill(ctx->have_dose.begin(), ctx->have_dose.end(), false);
     if (out) {
         out->n_segments = (int64_t)ctx->segments.size();
@@ -421,6 +431,27 @@ catch (...) { return on_exception(ctx); }
 // ------------------------------------------------------------------------------------------------------------------
 namespace {
 constexpr int kAuxStreams = 4;
+
+// per-phase launch table -> device (once per delivery simulation).  The tables live in pageable host memory, so the
+// copy goes through the H2D copy engine's queue: run_plan_host issues all of them BEFORE its bulk uploads, otherwise a
+// few KB needed by the first transport launch would wait behind gigabytes of CT and DVF traffic.
+int upload_segments(pbs4d_ctx* ctx, int phase, cudaStream_t st)
+{
+    const size_t np = ctx->launches.size();
+    if (ctx->seg_phase.size() < np) ctx->seg_phase.resize(np);
+    for (auto& b : ctx->seg_phase) if (!b) b.reset(new DevBuf);
+    if (ctx->seg_resident.size() < np) ctx->seg_resident.resize(np, false);
+    PhaseLaunch& L = ctx->launches[phase];
+    if (ctx->seg_resident[phase] || L.n_hist <= 0) return PBS4D_OK;
+    DevBuf& sb = *ctx->seg_phase[phase];
+    const size_t seg_bytes = L.segs.size() * sizeof(DevSegment);
+    CU(sb.ensure(seg_bytes + L.segs.size() * sizeof(long long)));
+    CU(cudaMemcpyAsync(sb.p, L.segs.data(), seg_bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(sb.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
+                       cudaMemcpyHostToDevice, st));
+    ctx->seg_resident[phase] = true;
+    return PBS4D_OK;
+}
 }
 
 extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* phases, uint64_t seed, double per_protons,
@@ -446,9 +477,9 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
         ctx->aux.resize(kAuxStreams, nullptr);
         for (auto& st : ctx->aux) CU(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
     }
-    if (ctx->seg_phase.size() < (size_t)ctx->n_phases) {
-        ctx->seg_phase.resize(ctx->n_phases);
-        for (auto& b : ctx->seg_phase) if (!b) b.reset(new DevBuf);
+    for (int a = 0; a < n; ++a) {                        // launch tables (no-op when run_plan_host uploaded them already)
+        const int urc = upload_segments(ctx, phases[a], ctx->stream);
+        if (urc != PBS4D_OK) return urc;
     }
     CU(ctx->counters.ensure(sizeof(TransportCounters) * 32));
     CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(TransportCounters) * n, ctx->stream));
@@ -471,16 +502,14 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
         guard(ctx->dose[phase]->ensure(nvox * sizeof(float)), "alloc dose grid");
         if (rc != PBS4D_OK) break;
         guard(cudaMemsetAsync(ctx->q[phase]->p, 0, nvox * sizeof(long long), st), "memset");
+        if (ctx->rho_pending[phase]) {                   // density still being produced on the copy stream
+            guard(cudaStreamWaitEvent(st, ctx->rho_ready[phase], 0), "wait for density");
+            ctx->rho_pending[phase] = false;
+        }
         guard(cudaEventRecord(ev[2 * a], st), "record");
         if (L.n_hist > 0) {
-            DevBuf& sb = *ctx->seg_phase[phase];
+            DevBuf& sb = *ctx->seg_phase[phase];          // uploaded on the context's stream before the fork
             const size_t seg_bytes = L.segs.size() * sizeof(DevSegment);
-            guard(sb.ensure(seg_bytes + L.segs.size() * sizeof(long long)), "alloc segments");
-            if (rc != PBS4D_OK) break;
-            guard(cudaMemcpyAsync(sb.p, L.segs.data(), seg_bytes, cudaMemcpyHostToDevice, st), "segments H2D");
-            guard(cudaMemcpyAsync(sb.as<char>() + seg_bytes, L.seg_begin.data(), L.segs.size() * sizeof(long long),
-                                  cudaMemcpyHostToDevice, st), "segments H2D");
-            guard(cudaEventRecord(ev[2 * a], st), "record");
             int64_t h0 = 0, hn = 0;
             pbs4d_shard_window(L.n_hist, ctx->shard_rank, ctx->shard_world, &h0, &hn);
             if (hn > 0)
@@ -838,51 +867,78 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     uint64_t bytes = 0;
     const pbs4d_grid& g = dose_grid ? *dose_grid : *ct;
     reset_phase_state(ctx, n_phases, g);
+    for (int p : active) {                               // launch tables first: see upload_segments
+        rc = upload_segments(ctx, p, ctx->stream);
+        if (rc != PBS4D_OK) return rc;
+    }
     const size_t ct_vox = (size_t)ct->nx * ct->ny * ct->nz;
     DevBuf& hu_dev = ctx->host_hu;
     CU(hu_dev.ensure(active.size() * ct_vox * sizeof(int16_t)));
     CU(ctx->table.ensure(2 * n_pts * sizeof(float)));
     // an early error return must not leave copies from the caller's host buffers in flight: armed before the first copy
     struct CopyGuard {
-        cudaStream_t st[2] = { nullptr, nullptr }; cudaEvent_t ev = nullptr; bool armed = false;
-        ~CopyGuard() { if (armed) { cudaStreamSynchronize(st[0]); cudaStreamSynchronize(st[1]); } if (ev) cudaEventDestroy(ev); }
+        cudaStream_t st[3] = { nullptr, nullptr, nullptr }; cudaEvent_t ev = nullptr; bool armed = false;
+        ~CopyGuard() { if (armed) for (auto s : st) cudaStreamSynchronize(s); if (ev) cudaEventDestroy(ev); }
     } guard;
-    if (disp_host && !ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
-    guard.st[0] = ctx->stream; guard.st[1] = ctx->copy_stream; guard.armed = true;
-    CU(cudaMemcpyAsync(ctx->table.p, hu_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
-    CU(cudaMemcpyAsync(ctx->table.as<float>() + n_pts, rho_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    if (!ctx->prep_stream) CU(cudaStreamCreateWithFlags(&ctx->prep_stream, cudaStreamNonBlocking));
+    guard.st[0] = ctx->stream; guard.st[1] = ctx->copy_stream; guard.st[2] = ctx->prep_stream; guard.armed = true;
+    // Host -> device traffic is pure DMA on the copy stream, back to back: the CT of every active phase, then the DVFs
+    // (each into its own staging area).  The kernels that consume an upload (HU -> density, DVF re-layout) run on a
+    // second stream behind per-upload events, so a kernel that has to wait for SM space under a running transport
+    // kernel never holds up the next copy.  The transport launch of a phase waits for that phase's density event only
+    // (mc_dose_phases): the first phase starts after its own 84 MB, everything else runs underneath the transport.
+    if (ctx->rho_ready.size() < (size_t)n_phases) ctx->rho_ready.resize(n_phases, nullptr);
+    if (ctx->upload_done.size() < (size_t)2 * n_phases) ctx->upload_done.resize((size_t)2 * n_phases, nullptr);
+    auto event_at = [&](std::vector<cudaEvent_t>& v, size_t i) -> cudaError_t {
+        return v[i] ? cudaSuccess : cudaEventCreateWithFlags(&v[i], cudaEventDisableTiming);
+    };
+    CU(cudaMemcpyAsync(ctx->table.p, hu_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
+    CU(cudaMemcpyAsync(ctx->table.as<float>() + n_pts, rho_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice,
+                       ctx->copy_stream));
     for (size_t a = 0; a < active.size(); ++a) {
         const int p = active[a];
         int16_t* dst = hu_dev.as<int16_t>() + a * ct_vox;
-        CU(cudaMemcpyAsync(dst, hu_host[p], ct_vox * sizeof(int16_t), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaMemcpyAsync(dst, hu_host[p], ct_vox * sizeof(int16_t), cudaMemcpyHostToDevice, ctx->copy_stream));
         bytes += ct_vox * sizeof(int16_t);
+        CU(event_at(ctx->upload_done, 2 * p));
+        CU(cudaEventRecord(ctx->upload_done[2 * p], ctx->copy_stream));
         CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
+        CU(cudaStreamWaitEvent(ctx->prep_stream, ctx->upload_done[2 * p], 0));
         launch_hu_to_density(*ct, dst, dose_grid, n_pts, ctx->table.as<float>(), ctx->table.as<float>() + n_pts,
-                             ctx->rho[p]->as<float>(), ctx->stream);
-        ctx->rho_valid[p] = true;
+                             ctx->rho[p]->as<float>(), ctx->prep_stream);
+        CU(event_at(ctx->rho_ready, p));
+        CU(cudaEventRecord(ctx->rho_ready[p], ctx->prep_stream));
+        ctx->rho_valid[p] = true; ctx->rho_pending[p] = true;
     }
     CU(cudaGetLastError());
     ctx->have_density = true;
-    // DVFs are not needed before the accumulation: their upload (the bulk of the host->device bytes) and re-layout
-    // run on a copy stream underneath the transport kernels
+    // DVFs are not needed before the accumulation (the bulk of the host->device bytes)
     cudaEvent_t& dvf_ready = guard.ev;
     if (disp_host) {
         const size_t dvf_vox = (size_t)dvf_grid->nx * dvf_grid->ny * dvf_grid->nz;
+        size_t n_dvf = 0;
+        for (int p : active) n_dvf += (p != ref_phase && disp_host[p]) ? 1 : 0;
         DevBuf& tmp = ctx->host_dvf;
-        CU(tmp.ensure(3 * dvf_vox * sizeof(float)));
+        CU(tmp.ensure(std::max<size_t>(n_dvf, 1) * 3 * dvf_vox * sizeof(float)));
+        size_t k = 0;
         for (int p : active) {
             if (p == ref_phase || !disp_host[p]) continue;
             auto& d = ctx->dvf[p];
             if (!d.disp) d.disp.reset(new DevBuf);
             CU(d.disp->ensure(4 * dvf_vox * sizeof(float)));
-            CU(cudaMemcpyAsync(tmp.p, disp_host[p], 3 * dvf_vox * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
+            float* stage = tmp.as<float>() + k * 3 * dvf_vox; ++k;
+            CU(cudaMemcpyAsync(stage, disp_host[p], 3 * dvf_vox * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
             bytes += 3 * dvf_vox * sizeof(float);
-            launch_dvf_interleave(*dvf_grid, tmp.as<float>(), d.disp->as<float>(), ctx->copy_stream);
+            CU(event_at(ctx->upload_done, 2 * p + 1));
+            CU(cudaEventRecord(ctx->upload_done[2 * p + 1], ctx->copy_stream));
+            CU(cudaStreamWaitEvent(ctx->prep_stream, ctx->upload_done[2 * p + 1], 0));
+            launch_dvf_interleave(*dvf_grid, stage, d.disp->as<float>(), ctx->prep_stream);
             d.set = true; d.ref = ref_phase; d.grid = *dvf_grid;
         }
         CU(cudaGetLastError());
         CU(cudaEventCreateWithFlags(&dvf_ready, cudaEventDisableTiming));
-        CU(cudaEventRecord(dvf_ready, ctx->copy_stream));
+        CU(cudaEventRecord(dvf_ready, ctx->prep_stream));
     }
     const auto t2 = clk::now();
 
