@@ -214,6 +214,9 @@ __device__ __forceinline__ void flush(const Params& P, Lane& L, long long& q_dep
     L.pend = 0;
 }
 
+// kMcs / kStrag: Highland deflection / Bohr straggling compiled in (the production kernel has both; the other three
+// instantiations serve the test switches PBS4D_NO_MCS / PBS4D_NO_STRAGGLE without flag tests in the step loop)
+template <bool kMcs, bool kStrag>
 __global__ void __launch_bounds__(kThreads, 4)
 transport_kernel(const __grid_constant__ Params P)
 {
@@ -229,7 +232,6 @@ transport_kernel(const __grid_constant__ Params P)
     uint32_t n_steps = 0, n_red = 0;                    // shared memory; per-step ones stay in registers
     const float hx = P.g.hx, hy = P.g.hy, hz = P.g.hz;
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
-    const bool do_mcs = !(P.flags & PBS4D_NO_MCS), do_strag = !(P.flags & PBS4D_NO_STRAGGLE);
 
     // Per-warp pool of 32 pre-sampled histories (T3 done by the whole warp at once, at full lane efficiency); a lane
     // whose history ends pops the next one instead of sampling it alone while 31 lanes wait.
@@ -352,7 +354,7 @@ transport_kernel(const __grid_constant__ Params P)
             uint32_t r0, r1, r2, r3;
             philox(P, L.m, L.g_lo, L.g_hi, r0, r1, r2, r3);
             float dE = dEm;
-            if (do_strag) {
+            if (kStrag) {
                 const float V2 = fmaf(fm, Bm.z - Am.z, Am.z);
                 const float a3 = angle_from_word(r3);
                 dE = fmaf(fast_sqrt(-V2 * t * fast_log2(u01(r2))), -__cosf(a3), dEm);
@@ -376,7 +378,7 @@ transport_kernel(const __grid_constant__ Params P)
 
             // T9: Highland deflection at the end of the step (kinematics at Em), branch-free orthonormal basis;
             // theta^2 = T t (-2 ln u0); sin and cos of the (small) polar angle by their Taylor polynomials
-            if (do_mcs) {
+            if (kMcs) {
                 const float T2  = fmaf(fm, Bm.w - Am.w, Am.w);
                 const float th2 = -T2 * t * fast_log2(u01(r0));
                 const float th  = fast_sqrt(th2);
@@ -439,13 +441,17 @@ transport_kernel(const __grid_constant__ Params P)
 
 }  // namespace
 
-const void* transport_kernel_symbol() { return (const void*)transport_kernel; }
+const void* transport_kernel_symbol() { return (const void*)transport_kernel<true, true>; }
 
 cudaError_t configure_transport(void)
 {
     // 22.5 KB table + 10 KB history pools per CTA: ask for a shared-memory carve-out that keeps 4 CTAs resident.
     // A per-device attribute: pbs4d_create calls this once for every context (any device).
-    return cudaFuncSetAttribute(transport_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+    cudaError_t e = cudaFuncSetAttribute(transport_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(transport_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(transport_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(transport_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 75);
+    return e;
 }
 
 size_t physics_table_bytes(void) { return sizeof(TabNode) * kTabNodes; }
@@ -460,14 +466,17 @@ void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* s
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
     P.Q = (unsigned long long*)Q; P.counters = counters;
+    const bool mcs = !(flags & PBS4D_NO_MCS), strag = !(flags & PBS4D_NO_STRAGGLE);
+    void (*kernel)(const Params) = mcs ? (strag ? transport_kernel<true, true> : transport_kernel<true, false>)
+                                       : (strag ? transport_kernel<false, true> : transport_kernel<false, false>);
     int per_sm = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, transport_kernel, kThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0);
     if (per_sm < 1) per_sm = 1;
     long long want = (n_hist + kThreads - 1) / kThreads;
     long long cap  = (long long)sm_count * per_sm;
     int blocks = (int)(want < cap ? want : cap);
     if (blocks < 1) blocks = 1;
-    transport_kernel<<<blocks, kThreads, 0, st>>>(P);
+    kernel<<<blocks, kThreads, 0, st>>>(P);
 }
 
 }  // namespace pbs4d
