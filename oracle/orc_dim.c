@@ -4,7 +4,9 @@
  *    subvoxel r_ik was mapped to I_S giving T^{R->S}(r_ik), the trilinearly-interpolated dose at this location
  *    D~^S[T^{R->S}(r_ik)] was computed and the final D_i^S was then  D_i^S = n^-3 sum_k D~^S[T^{R->S}(r_ik)]".
  * Steps (DESIGN.md "DIM steps" P1-P5; arithmetic as for the EMTM oracle: strict IEEE fp32, one rounding per
- * operation, no fused multiply-add; the sum over subvoxels in double, in (c, b, a) loop order):
+ * operation, no fused multiply-add; the sum over subvoxels in double, in (b, a, c) loop order -- c, the z index,
+ * innermost: Eq. 3 is a plain mean, the paper fixes no order, and this one lets an implementation walk a subvoxel
+ * column along z, where consecutive subvoxels share the x/y-interpolated DVF values (reading D4)):
  *   P1  subvoxel centre on the reference grid            p = o + ((float)i + (a + 0.5f)/ns) * h      (as A2)
  *   P2  displacement T^{R->S} at p by trilinear interpolation between DVF-grid centres (as A3);
  *       a centre outside the DVF grid's voxel extent contributes nothing
@@ -81,9 +83,9 @@ int orc_dim_pull(const orc_grid* R, int32_t nsx, int32_t nsy, int32_t nsz,
     for (int j = 0; j < R->ny; ++j)
     for (int i = 0; i < R->nx; ++i) {
         double sum = 0.0;
-        for (int c = 0; c < nsz; ++c)
         for (int b = 0; b < nsy; ++b)
-        for (int a = 0; a < nsx; ++a) {
+        for (int a = 0; a < nsx; ++a)
+        for (int c = 0; c < nsz; ++c) {
             n_sub += 1;
             /* P1 */
             float p[3] = { centre_of(R->ox, R->hx, i, a, nsx), centre_of(R->oy, R->hy, j, b, nsy),
