@@ -382,6 +382,7 @@ struct PullParams {
     const float* __restrict__ dose;          // source-phase dose on grid src
     double* acc;                             // [ref voxels]
     int nsx, nsy, nsz;
+    int chunk_z;                             // reference voxels along z handled by one thread
     AccCounters* counters;
 };
 
@@ -400,6 +401,13 @@ __device__ __forceinline__ Cell cell_of(float p, float o, float h, int n)
     return c;
 }
 
+// Thread = a column of chunk_z reference voxels at (i, j); CTA = 32 x 4 columns.  Loop nest as in the push: subvoxel
+// (b, a) of the column outside, all its z-subvoxels inside, so that the x/y-lerps of the DVF interpolation are
+// evaluated once per z-NODE (the upper node of a cell is the lower node of the next) and the "new z-cell" branch is
+// warp-uniform.  The double sum of a voxel receives its values in (b, a, c) order -- reading D4 -- because every voxel
+// of the column keeps its own running sum (shared memory) and the c-run of a (b, a) column is added to it value by
+// value.  Per subvoxel: z-lerp, q = r + u, the source-grid cell of q (three IEEE divisions: the continuous index is
+// needed as a value, not only its floor), 8 dose loads, 7 lerps, one double add.
 __global__ void __launch_bounds__(kTileX * kTileY)
 dim_pull_kernel(const __grid_constant__ PullParams P)
 {
@@ -407,12 +415,14 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
     AxisEntry* sx = s_map;
     AxisEntry* sy = sx + kTileX * P.nsx;
     AxisEntry* sz = sy + kTileY * P.nsy;
+    double* s_sum = reinterpret_cast<double*>(sz + P.chunk_z * P.nsz);       // [chunk_z][128] running sums
     const int tid = threadIdx.y * kTileX + threadIdx.x;
     const int i = blockIdx.x * kTileX + threadIdx.x;
     const int j = blockIdx.y * kTileY + threadIdx.y;
-    const int k = blockIdx.z;
-    const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy;
-    for (int e = tid; e < n_x + n_y + P.nsz; e += kTileX * kTileY) {
+    const int k0 = blockIdx.z * P.chunk_z;
+    const int kz_n = min(P.chunk_z, P.ref.nz - k0);
+    const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy, n_z = kz_n * P.nsz;
+    for (int e = tid; e < n_x + n_y + n_z; e += kTileX * kTileY) {
         if (e < n_x)
             s_map[e] = axis_map(P.ref.ox, P.ref.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
                                 P.dvf.ox, P.dvf.hx, P.dvf.nx);
@@ -420,8 +430,10 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
             s_map[e] = axis_map(P.ref.oy, P.ref.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
                                 P.dvf.oy, P.dvf.hy, P.dvf.ny);
         else
-            s_map[e] = axis_map(P.ref.oz, P.ref.hz, k, e - n_x - n_y, P.nsz, P.dvf.oz, P.dvf.hz, P.dvf.nz);
+            sz[e - n_x - n_y] = axis_map(P.ref.oz, P.ref.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
+                                         P.dvf.oz, P.dvf.hz, P.dvf.nz);
     }
+    for (int kk = 0; kk < kz_n; ++kk) s_sum[kk * (kTileX * kTileY) + tid] = 0.0;
     __syncthreads();
 
     unsigned n_src = 0, n_dvf = 0;
@@ -433,51 +445,58 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
         const float sox = P.src.ox, soy = P.src.oy, soz = P.src.oz, shx = P.src.hx, shy = P.src.hy, shz = P.src.hz;
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * nsy;
-        double sum = 0.0;
-        for (int c = 0; c < nsz; ++c) {
-            const AxisEntry mz = sz[c];
-            for (int b = 0; b < nsy; ++b) {
-                const AxisEntry my = syl[b];
-                const int r00 = (mz.i0 * dny + my.i0) * dnx;
-                const int sy1 = (my.flags & 1) * dnx, sz1 = (mz.flags & 1) * dny * dnx;
-                const float4* __restrict__ p00 = P.U + r00;
-                const float4* __restrict__ p01 = p00 + sy1;
-                const float4* __restrict__ p10 = p00 + sz1;
-                const float4* __restrict__ p11 = p10 + sy1;
-                const bool ok_zy = (mz.flags & my.flags & 2) != 0;
-                for (int a = 0; a < nsx; ++a) {
-                    const AxisEntry mx = sxl[a * kTileX];
-                    if (!(ok_zy && (mx.flags & 2))) { n_dvf += 1; continue; }
-                    const int x0 = mx.i0;
-                    const float4 a000 = __ldg(p00 + x0), a001 = __ldg(p00 + x0 + dx1);
-                    const float4 a010 = __ldg(p01 + x0), a011 = __ldg(p01 + x0 + dx1);
-                    const float4 a100 = __ldg(p10 + x0), a101 = __ldg(p10 + x0 + dx1);
-                    const float4 a110 = __ldg(p11 + x0), a111 = __ldg(p11 + x0 + dx1);
-#define PBS4D_TRILERP(cmp) lerp_rn(lerp_rn(lerp_rn(a000.cmp, a001.cmp, mx.w), lerp_rn(a010.cmp, a011.cmp, mx.w), my.w), \
-                                   lerp_rn(lerp_rn(a100.cmp, a101.cmp, mx.w), lerp_rn(a110.cmp, a111.cmp, mx.w), my.w), mz.w)
-                    const float qx = __fadd_rn(mx.p, PBS4D_TRILERP(x));
-                    const float qy = __fadd_rn(my.p, PBS4D_TRILERP(y));
-                    const float qz = __fadd_rn(mz.p, PBS4D_TRILERP(z));
-#undef PBS4D_TRILERP
-                    const Cell cx = cell_of(qx, sox, shx, snx), cy = cell_of(qy, soy, shy, sny),
-                               cz = cell_of(qz, soz, shz, snz);
-                    if (!(cx.ok && cy.ok && cz.ok)) { n_src += 1; continue; }
-                    const float* __restrict__ d00 = P.dose + ((size_t)cz.i0 * sny + cy.i0) * snx + cx.i0;
-                    const float* __restrict__ d01 = d00 + cy.d1 * snx;
-                    const float* __restrict__ d10 = d00 + (size_t)cz.d1 * sny * snx;
-                    const float* __restrict__ d11 = d10 + cy.d1 * snx;
-                    const float c00 = lerp_rn(__ldg(d00), __ldg(d00 + cx.d1), cx.w);
-                    const float c01 = lerp_rn(__ldg(d01), __ldg(d01 + cx.d1), cx.w);
-                    const float c10 = lerp_rn(__ldg(d10), __ldg(d10 + cx.d1), cx.w);
-                    const float c11 = lerp_rn(__ldg(d11), __ldg(d11 + cx.d1), cx.w);
-                    const float val = lerp_rn(lerp_rn(c00, c01, cy.w), lerp_rn(c10, c11, cy.w), cz.w);
-                    sum = __dadd_rn(sum, (double)val);
+        const int sz_stride = dny * dnx;
+        for (int b = 0; b < nsy; ++b) {
+            const AxisEntry my = syl[b];
+            const int sy1 = (my.flags & 1) * dnx;
+            for (int a = 0; a < nsx; ++a) {
+                const AxisEntry mx = sxl[a * kTileX];
+                if (!(mx.flags & my.flags & 2)) { n_dvf += (unsigned)n_z; continue; }      // column outside the DVF extent
+                const float4* __restrict__ col = P.U + my.i0 * dnx + mx.i0;
+                int node_hi = -1, cell_z = -1;
+                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f, ddx = 0.f, ddy = 0.f, ddz = 0.f;
+                const AxisEntry* mzp = sz;
+                for (int kk = 0; kk < kz_n; ++kk) {
+                    double sum = s_sum[kk * (kTileX * kTileY) + tid];
+                    for (int c = 0; c < nsz; ++c, ++mzp) {
+                        const AxisEntry mz = *mzp;
+                        if (!(mz.flags & 2)) { n_dvf += 1; continue; }                     // warp-uniform
+                        if (mz.i0 != cell_z) {                                             // new DVF z-cell (uniform)
+                            cell_z = mz.i0;
+                            const int hi = mz.i0 + (mz.flags & 1);
+                            if (mz.i0 == node_hi) { c0x = c1x; c0y = c1y; c0z = c1z; }
+                            else bilerp3(load_quad(col + (size_t)mz.i0 * sz_stride, dx1, sy1), mx.w, my.w, c0x, c0y, c0z);
+                            if (hi == mz.i0) { c1x = c0x; c1y = c0y; c1z = c0z; }
+                            else bilerp3(load_quad(col + (size_t)hi * sz_stride, dx1, sy1), mx.w, my.w, c1x, c1y, c1z);
+                            node_hi = hi;
+                            ddx = __fsub_rn(c1x, c0x); ddy = __fsub_rn(c1y, c0y); ddz = __fsub_rn(c1z, c0z);
+                        }
+                        const float qx = __fadd_rn(mx.p, __fadd_rn(c0x, __fmul_rn(mz.w, ddx)));
+                        const float qy = __fadd_rn(my.p, __fadd_rn(c0y, __fmul_rn(mz.w, ddy)));
+                        const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, ddz)));
+                        const Cell cx = cell_of(qx, sox, shx, snx), cy = cell_of(qy, soy, shy, sny),
+                                   cz = cell_of(qz, soz, shz, snz);
+                        if (!(cx.ok && cy.ok && cz.ok)) { n_src += 1; continue; }
+                        const float* __restrict__ d00 = P.dose + ((size_t)cz.i0 * sny + cy.i0) * snx + cx.i0;
+                        const float* __restrict__ d01 = d00 + cy.d1 * snx;
+                        const float* __restrict__ d10 = d00 + (size_t)cz.d1 * sny * snx;
+                        const float* __restrict__ d11 = d10 + cy.d1 * snx;
+                        const float c00 = lerp_rn(__ldg(d00), __ldg(d00 + cx.d1), cx.w);
+                        const float c01 = lerp_rn(__ldg(d01), __ldg(d01 + cx.d1), cx.w);
+                        const float c10 = lerp_rn(__ldg(d10), __ldg(d10 + cx.d1), cx.w);
+                        const float c11 = lerp_rn(__ldg(d11), __ldg(d11 + cx.d1), cx.w);
+                        const float val = lerp_rn(lerp_rn(c00, c01, cy.w), lerp_rn(c10, c11, cy.w), cz.w);
+                        sum = __dadd_rn(sum, (double)val);
+                    }
+                    s_sum[kk * (kTileX * kTileY) + tid] = sum;
                 }
             }
         }
-        const size_t v = ((size_t)k * P.ref.ny + j) * P.ref.nx + i;
         const double n3 = __dmul_rn(__dmul_rn((double)nsx, (double)nsy), (double)nsz);
-        P.acc[v] = __dadd_rn(P.acc[v], __ddiv_rn(sum, n3));
+        for (int kk = 0; kk < kz_n; ++kk) {
+            const size_t v = ((size_t)(k0 + kk) * P.ref.ny + j) * P.ref.nx + i;
+            P.acc[v] = __dadd_rn(P.acc[v], __ddiv_rn(s_sum[kk * (kTileX * kTileY) + tid], n3));
+        }
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
@@ -516,7 +535,9 @@ cudaError_t configure_accumulate(void)
 {
     // the push kernel's axis maps + per-voxel (e_q, m_q) stage need up to 57 KB of dynamic shared memory at 64
     // subvoxels per axis.  A per-device attribute: pbs4d_create calls this for every context.
-    return cudaFuncSetAttribute(emtm_push_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(emtm_push_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dim_pull_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    return e;
 }
 
 void launch_dvf_interleave(const pbs4d_grid& g, const float* disp_planar, float* out4, cudaStream_t st)
@@ -591,9 +612,12 @@ void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs
     PullParams P;
     P.ref = ref; P.dvf = dvf_grid; P.src = src; P.U = reinterpret_cast<const float4*>(disp4); P.dose = dose_src;
     P.acc = acc; P.nsx = nsx; P.nsy = nsy; P.nsz = nsz; P.counters = counters;
-    dim3 b(kTileX, kTileY, 1), g((ref.nx + kTileX - 1) / kTileX, (ref.ny + kTileY - 1) / kTileY, ref.nz);
-    const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + nsz) * sizeof(AxisEntry);
-    dim_pull_kernel<<<g, b, smem, st>>>(P);
+    P.chunk_z = nsz <= 2 ? kChunkZMax : 4;               // as for the push: longer columns amortise the first z-node
+    dim3 b(kTileX, kTileY, 1), g((ref.nx + kTileX - 1) / kTileX, (ref.ny + kTileY - 1) / kTileY,
+                                 (ref.nz + P.chunk_z - 1) / P.chunk_z);
+    const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
+                        (size_t)P.chunk_z * kTileX * kTileY * sizeof(double);
+    dim_pull_kernel<<<g, b, smem, st>>>(P);              // <= 52 KB: configure_accumulate() opted in
 }
 
 void launch_dim_final(const pbs4d_grid& ref, int n_src, const pbs4d_grid* dvf_grids_host, const double* acc,

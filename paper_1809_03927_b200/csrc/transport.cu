@@ -298,10 +298,13 @@ transport_kernel(const __grid_constant__ Params P)
                 exhausted = true;                       // pool empty and nothing left to fetch
             }
         }
-        if (!__any_sync(0xffffffffu, alive)) {
+        const unsigned live = __ballot_sync(0xffffffffu, alive);
+        if (live == 0u) {
             if (__all_sync(0xffffffffu, exhausted)) break;
             continue;
         }
+        // step loop: one vote per iteration; it is left as soon as a lane's history ends (back to the refill phase)
+        do {
         if (alive) {
             // ---------------- one condensed-history step (T5-T10) ----------------
             L.m += 1u;
@@ -416,6 +419,7 @@ transport_kernel(const __grid_constant__ Params P)
                 }
             }
         }
+        } while (__ballot_sync(0xffffffffu, alive) == live);
     }
 
     // block-level tally reduction: warp shuffle, shared atomics, one global atomic per block and counter
