@@ -175,3 +175,28 @@ def test_bench_pass_sharded_equals_single(ctx):
         n, out, st = bench.run_pass(ctx, cfg, hu_dev, dvf_dev, r, world, sum_grids=all_reduce_stub, share=broadcast_stub)
         assert torch.equal(out.view(torch.int32), out1.view(torch.int32)), f"rank {r}"
         assert st["launches"] > 0 and st["phases"] == st1["phases"]
+
+
+def test_call_order_and_argument_errors_of_the_split_calls(ctx):
+    cfg = synth.config3(div=4, n_hist=20_000)
+    phases, deliv = setup(ctx, cfg)
+    ref = cfg["ref_phase"]
+    with pytest.raises(RuntimeError, match="mc_dose_phase not run"):
+        ctx.phase_energy_view(phases[0])                       # no transport yet for this delivery
+    with pytest.raises(RuntimeError, match="mc_dose_phase not run"):
+        ctx.finalize_phase_dose(phases[0])
+    ctx.mc_dose_phases(phases, cfg["seed"])
+    with pytest.raises(RuntimeError, match="not pushed|no accumulators"):
+        ctx.accumulate_finalize(ref)                           # a9 before any a8
+    with pytest.raises(RuntimeError):
+        ctx.accumulator_views(ref)                             # the reference phase has no accumulators
+    st = ctx.accumulate_push(ref, cfg["subvox"], 0)            # empty mask: nothing pushed, everything zeroed
+    assert st["subvoxels"] == 0
+    out, _ = ctx.accumulate_finalize(ref)                      # = the reference dose inside the DVF coverage
+    d_ref = ctx.mc_dose_phase(ref, cfg["seed"])[0]
+    inside = out != 0
+    assert int(inside.sum()) > 0 and torch.equal(out[inside], d_ref[inside])
+    with pytest.raises(RuntimeError):
+        ctx.accumulate_push(ref, (0, 2, 2), 1)
+    with pytest.raises(RuntimeError):
+        ctx.phase_energy_view(99)
