@@ -23,12 +23,46 @@ namespace pbs4d {
 
 namespace {
 
+// ---- packed fp32 pairs (sm_100 f32x2: ONE issue slot for two individually rounded fp32 operations) ----
+// The push is bound by instruction issue, not by the FP32 pipe, so the x and y components --
+// and the two ends of a rounding interval -- travel as a pair through add/sub/mul/fma.rn.f32x2 (SASS FADD2 / FMUL2 /
+// FFMA2).  Each half is the IEEE round-to-nearest result of its own operation, exactly as the scalar intrinsic gives.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi)
+{
+    f32x2 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d;
+}
+__device__ __forceinline__ void upk(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+
 // One axis of the subvoxel -> DVF-cell map (A2, A3): subvoxel centre p, lower DVF node i0, upper node i0 + d1,
 // weight w, and whether the centre lies inside the DVF grid's voxel extent.  It depends on (voxel index, subvoxel
 // index) of that axis only, so a CTA computes it once per axis for its tile and keeps it in shared memory.
-struct __align__(16) AxisEntry { float p, w; int i0; int flags; };      // flags: bit0 = d1, bit1 = ok
+// P = RN_f32((p - o_ref) (1 / h_ref) - 0.5) in double: the centre's continuous reference-grid index minus one half,
+// the constant term of the push kernel's folded index estimate (fast path only; never enters a contract value).
+struct __align__(16) AxisEntry { float p, w, P; int cell; };            // cell: i0 | d1 << 29 | ok << 30
+constexpr int kCellD1 = 1 << 29, kCellOk = 1 << 30, kCellNode = kCellD1 - 1;
 
-__device__ __forceinline__ AxisEntry axis_map(float o, float h, int i, int a, int ns, float od, float hd, int nd)
+__device__ __forceinline__ AxisEntry axis_map(float o, float h, int i, int a, int ns, float od, float hd, int nd,
+                                              float o_ref, double inv_h_ref)
 {
     AxisEntry m;
     const float f = __fdiv_rn(__fadd_rn((float)a, 0.5f), (float)ns);
@@ -38,9 +72,9 @@ __device__ __forceinline__ AxisEntry axis_map(float o, float h, int i, int a, in
     g = fminf(fmaxf(g, 0.0f), (float)(nd - 1));
     int k = (int)floorf(g);
     k = max(min(k, nd - 2), 0);
-    m.i0 = k;
     m.w  = __fsub_rn(g, (float)k);
-    m.flags = (min(k + 1, nd - 1) - k) | (ok ? 2 : 0);
+    m.cell = k | ((min(k + 1, nd - 1) - k) ? kCellD1 : 0) | (ok ? kCellOk : 0);
+    m.P = (float)(((double)m.p - (double)o_ref) * inv_h_ref - 0.5);
     return m;
 }
 
@@ -48,29 +82,38 @@ __device__ __forceinline__ float lerp_rn(float A, float B, float w)
 {
     return __fadd_rn(A, __fmul_rn(w, __fsub_rn(B, A)));
 }
+// A + RN(w d) per half, two roundings.  ptxas (12.9) contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 even under
+// --fmad=false and with the explicit .rn, which would break the contract's operation-by-operation rounding; the
+// scalar mul.rn.f32 is never contracted, so the products are formed by two FMULs and only the add is packed.
+__device__ __forceinline__ f32x2 mad2_unfused(f32x2 A, float w, f32x2 d)
+{
+    float dl, dh;
+    upk(d, dl, dh);
+    return add2(A, pk(__fmul_rn(w, dl), __fmul_rn(w, dh)));
+}
+__device__ __forceinline__ f32x2 lerp2(f32x2 A, f32x2 B, float w)       // both halves: A + w (B - A), as lerp_rn
+{
+    return mad2_unfused(A, w, sub2(B, A));
+}
 
 // A4: ix = floorf((q - o) / h) with the IEEE quotient Q = RN(RN(q - o) / h), inside iff 0 <= ix < n.
-// Fast path (FMA/ALU pipes only, no division, no conversion instruction, no call):
-//   y = fma(q, inv_h, c),  inv_h = RN(1/h),  c = RN(-o inv_h - 0.5)      ~  Q - 0.5
-//   t = y + 1.5 2^23  rounds y to the nearest integer r = t - 1.5 2^23 (exact for |y| < 2^22), and r is also the
-//   difference of the bit patterns of t and 1.5 2^23.  Unless Q lies close to an integer, floor(Q) = r.
-// |y - (Q - 0.5)| <= 2^-24 (|Q| + |q inv_h| + |c| + |y|) + ulp(c)/2: the rounding of q - o that the contract
-// prescribes is a relative 2^-24 on Q, inv_h carries a relative 2^-24, c and y one rounding each.  The launcher
-// turns this into a per-axis tolerance tol = 4e-7 (n + 2 + 2 |o| / h); when fr = y - r is within tol of +-0.5, Q is
-// that close to an integer and the decision is taken exactly (exact_floor).  For |y| >= 2^22 (and +-Inf) the integer
-// comes out >= 2^22 - 1 or negative, i.e. outside every grid the fast path is used for (the launcher passes
-// tol = +Inf -- always exact -- when a reference dimension exceeds 4e6); NaN fails the comparison and goes exact.
+// The push kernel does not form Q on its main path.  It evaluates an ESTIMATE y of Q - 0.5 with the z-lerp, q = p + u
+// and the division folded into one fma per axis (see emtm_push_kernel), rounds it to the nearest integer r with the
+// 1.5 2^23 trick, and accepts floor(Q) = r only when y is farther than tol from r +- 0.5, where tol bounds
+// |y - (Q - 0.5)|:
+//   contract   wd = RN(w dd), u = RN(c0 + wd), q = RN(p + u), e = RN(q - o), Q = RN(e / h):
+//              |Q - Qr| <= eps (|w dd| + |u| + |q| + |e|) / h + eps |Q|,    Qr the real-number value, eps = 2^-24
+//   estimate   B = RN(dd ih), A = RN(c0 ih + P), y = RN(w B + A), ih = RN(1 / h), P as in axis_map:
+//              |y - (Qr - 0.5)| <= eps (2 |w dd| / h + |c0| / h + |P| + |A| + |y|)
+// With |u|, |c0| <= U (largest nodal displacement of the field), |w dd| <= 2 U, |q| <= |o| + |e|, and |Q| <= n + 1:
+//   |y - (Q - 0.5)| <= eps (6 (n + 1) + 12 U / h + |o| / h + 2)            (z: the same count with one more rounding)
+// tol = 2 eps (8 (n + 2) + 16 U / h + 2 |o| / h), more than 2.5 times that.  Beyond |Q| = n + 1 the error grows by
+// 8 eps per unit of |Q|, so a point outside the grid stays outside.  A subvoxel that fails the test ("near") is
+// decided by the contract's own operations and exact_floor.  U is measured when the field is stored
+// (dvf_interleave_kernel); a field with non-finite displacements, tol >= 0.25 or a reference dimension above 4e6
+// (the range of the rounding trick) makes every subvoxel take the exact path.
 constexpr float kMagic     = 12582912.0f;          // 1.5 * 2^23
 constexpr int   kMagicBits = 0x4B400000;
-
-__device__ __forceinline__ bool fast_floor(float q, float inv_h, float c, float half_minus_tol, int& ix)
-{
-    const float y  = __fmaf_rn(q, inv_h, c);
-    const float t  = __fadd_rn(y, kMagic);
-    const float fr = __fsub_rn(y, __fsub_rn(t, kMagic));
-    ix = __float_as_int(t) - kMagicBits;
-    return !(fabsf(fr) <= half_minus_tol);         // true: Q is too close to an integer (or NaN) -> exact_floor
-}
 
 // Exact floorf(RN(e / h)) for e = RN(q - o), decided without a division instruction or subroutine (the kernel's
 // inner loop stays free of calls).  yq = RN(e inv_h) is within 2^-23 |yq| of Q = RN(e / h); k = the integer nearest
@@ -97,14 +140,37 @@ __device__ __forceinline__ int exact_floor(float e, float h, float inv_h, int n)
     return (unsigned)fl < (unsigned)n ? fl : -1;
 }
 
-// planar [3][N] displacement field -> one float4 {ux, uy, uz, 0} per DVF node, so that a trilinear corner is one
-// 128-bit load instead of three 32-bit loads
-__global__ void dvf_interleave_kernel(size_t n, const float* __restrict__ ux, const float* __restrict__ uy,
-                                      const float* __restrict__ uz, float4* __restrict__ out)
+// planar [3][N] displacement field -> one float4 {ux, uy, uz, uz of the y-neighbour} per DVF node: a trilinear corner
+// is one 128-bit load, (ux, uy) is a ready f32x2 pair, and (uz(y), uz(y + 1)) is the pair the x-lerp of the z component
+// works on, so the rows y0 + 1 are read as 64-bit (ux, uy) only.  The y-neighbour is clamped (ny == 1: itself), as the
+// axis map clamps the upper node.  The kernel also measures U = max |u| per component (out[n].xyz as bit patterns;
+// the ordering of non-negative floats is that of their bit patterns, NaN above Inf) for the push kernel's tolerance.
+__global__ void __launch_bounds__(128)
+dvf_interleave_kernel(int nx, int ny, const float* __restrict__ ux, const float* __restrict__ uy,
+                      const float* __restrict__ uz, float4* __restrict__ out)
 {
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-        out[i] = make_float4(ux[i], uy[i], uz[i], 0.0f);
+    const int row = blockIdx.x;                          // y + ny z
+    const int x = blockIdx.y * blockDim.x + threadIdx.x;
+    unsigned mx = 0u, my = 0u, mz = 0u;
+    if (x < nx) {
+        const size_t i = (size_t)row * nx + x;
+        const float a = ux[i], b = uy[i], c = uz[i];
+        out[i] = make_float4(a, b, c, (row % ny) + 1 < ny ? uz[i + nx] : c);
+        mx = __float_as_uint(fabsf(a)); my = __float_as_uint(fabsf(b)); mz = __float_as_uint(fabsf(c));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+        my = max(my, __shfl_xor_sync(0xffffffffu, my, off));
+        mz = max(mz, __shfl_xor_sync(0xffffffffu, mz, off));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        unsigned* u = reinterpret_cast<unsigned*>(out + (size_t)gridDim.x * nx);
+        // a (possibly stale, L1-cached) read first: after the first few warps nearly every warp skips the atomic
+        if (mx > u[0]) atomicMax(u + 0, mx);
+        if (my > u[1]) atomicMax(u + 1, my);
+        if (mz > u[2]) atomicMax(u + 2, mz);
+    }
 }
 
 constexpr int kTileX = 32, kTileY = 4, kChunkZMax = 8;
@@ -113,48 +179,180 @@ struct PushParams {
     pbs4d_grid src, dvf, ref;
     const float* __restrict__ dose;
     const float* __restrict__ rho;
-    const float4* __restrict__ U;            // interleaved DVF
+    const float4* __restrict__ U;            // interleaved DVF, U[nodes] = {max|ux|, max|uy|, max|uz|, -}
     float inv_hrx, inv_hry, inv_hrz;         // RN(1 / h) of the reference grid
-    float cx, cy, cz;                        // RN(-o inv_h - 0.5) per axis (fast_floor)
-    float htx, hty, htz;                     // 0.5 - tol per axis (fast_floor)
+    double ihdx, ihdy, ihdz;                 // 1 / h in double (axis_map's P)
+    float tgx, tgy, tgz;                     // geometric part of the index tolerance: 2^-23 (8 (n + 2) + 2 |o| / h)
+    float tux, tuy, tuz;                     // its slope in U: 2^-23 16 / h          (+Inf, 0: always exact)
     int nsx, nsy, nsz;
     int chunk_z;                             // source voxels along z handled by one thread (<= kChunkZMax)
+    int tile_cap;                            // DVF nodes the CTA's shared-memory tile can hold
     unsigned long long* E;
     unsigned long long* M;
     AccCounters* counters;
 };
 
-// the four DVF nodes (x0|x0+1, y0|y0+1) of one z-node that a subvoxel column interpolates between
-struct Quad { float4 a00, a01, a10, a11; };
-
-__device__ __forceinline__ Quad load_quad(const float4* __restrict__ p, int dx1, int sy1)
+// x- then y-interpolation of the three displacement components at one z-node (A3: 2 + 1 of the 7 lerps) from the four
+// corners of the float4 layout of dvf_interleave_kernel: 19 packed / scalar operations instead of 27.
+__device__ __forceinline__ void bilerp_corners(const float4& a00, const float4& a01, const float2& a10, const float2& a11,
+                                               float wx, float wy, f32x2& cxy, float& cz)
 {
-    Quad q;
-    q.a00 = __ldg(p); q.a01 = __ldg(p + dx1); q.a10 = __ldg(p + sy1); q.a11 = __ldg(p + sy1 + dx1);
-    return q;
+    const f32x2 r0 = lerp2(pk(a00.x, a00.y), pk(a01.x, a01.y), wx);
+    const f32x2 r1 = lerp2(pk(a10.x, a10.y), pk(a11.x, a11.y), wx);
+    cxy = lerp2(r0, r1, wy);
+    float z0, z1;
+    upk(lerp2(pk(a00.z, a00.w), pk(a01.z, a01.w), wx), z0, z1);         // uz rows y0 and y0 + 1 (a00.w = uz of row y0 + 1)
+    cz = lerp_rn(z0, z1, wy);
+}
+// p: node (x0, y0) of the z-node in global memory; dx1, sy1: offsets (in nodes) of the x- and y-neighbour
+__device__ __forceinline__ void node_bilerp(const float4* __restrict__ p, int dx1, int sy1, float wx, float wy,
+                                            f32x2& cxy, float& cz)
+{
+    bilerp_corners(__ldg(p), __ldg(p + dx1), __ldg(reinterpret_cast<const float2*>(p + sy1)),
+                   __ldg(reinterpret_cast<const float2*>(p + sy1 + dx1)), wx, wy, cxy, cz);
+}
+// the same from the CTA's shared-memory tile (x-neighbour = next node)
+__device__ __forceinline__ void node_bilerp_tile(const float4* p, int sy1, float wx, float wy, f32x2& cxy, float& cz)
+{
+    bilerp_corners(p[0], p[1], *reinterpret_cast<const float2*>(p + sy1), *reinterpret_cast<const float2*>(p + sy1 + 1),
+                   wx, wy, cxy, cz);
 }
 
-// x- then y-interpolation of the three displacement components at one z-node (A3: 2 + 1 of the 7 lerps)
-__device__ __forceinline__ void bilerp3(const Quad& q, float wx, float wy, float& cx, float& cy, float& cz)
+// DVF tile of a CTA in shared memory: nodes [x0, x0 + nx) x [y0, y0 + ny) x [z0, z0 + nz) of the field
+struct Tile { int x0, y0, z0, nx, ny, nz; };
+
+// The subvoxel columns of one thread.
+// kChecked = false: the CTA's source tile, displaced by at most U, lies at least one voxel inside the reference grid
+// on every axis and entirely inside the DVF grid's z-extent, so no destination can fall outside and the range test is
+// compiled out.  kTile: the DVF nodes come from the CTA's shared-memory tile instead of global memory.
+template <bool kChecked, bool kTile>
+__device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntry* __restrict__ sxl,
+                                             const AxisEntry* __restrict__ syl, const AxisEntry* __restrict__ sz,
+                                             const longlong2* __restrict__ s_em_t, const float4* tile, const Tile T,
+                                             int kz_n, int okz, float htx, float hty, f32x2 tolz12, unsigned& eligible,
+                                             unsigned& landed)
 {
-    cx = lerp_rn(lerp_rn(q.a00.x, q.a01.x, wx), lerp_rn(q.a10.x, q.a11.x, wx), wy);
-    cy = lerp_rn(lerp_rn(q.a00.y, q.a01.y, wx), lerp_rn(q.a10.y, q.a11.y, wx), wy);
-    cz = lerp_rn(lerp_rn(q.a00.z, q.a01.z, wx), lerp_rn(q.a10.z, q.a11.z, wx), wy);
+    const int nsx = P.nsx, nsy = P.nsy, nsz = P.nsz;
+    const int dnx = P.dvf.nx;
+    const int dx1 = dnx > 1 ? 1 : 0;                     // upper x node = lower + 1 unless the DVF grid is 1 node wide
+    const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
+    const int sz_stride = kTile ? T.ny * T.nx : P.dvf.ny * dnx;
+    const int row = kTile ? T.nx : dnx;
+    // destination index from the bit patterns b = kMagicBits + index of the rounded estimates:
+    // (bz rny + by) rnx + bx = dst + kShift (mod 2^32); kNone is the shifted "no destination"
+    const unsigned kShift = (unsigned)kMagicBits * ((unsigned)rny * (unsigned)rnx + (unsigned)rnx + 1u), kNone = kShift - 1u;
+    const f32x2 ihxy = pk(P.inv_hrx, P.inv_hry), ihzz = pk(P.inv_hrz, P.inv_hrz);
+    const f32x2 magic2 = pk(kMagic, kMagic);
+    for (int b = 0; b < nsy; ++b) {
+        const AxisEntry my = syl[b];
+        const int sy1 = (my.cell & kCellD1) ? row : 0;
+        for (int a = 0; a < nsx; ++a) {
+            const AxisEntry mx = sxl[a * kTileX];
+            if (!(mx.cell & my.cell & kCellOk)) continue;                         // whole column outside the DVF extent
+            eligible += (unsigned)okz;
+            // node (x0, y0) of z-node 0 of the field (global) or of the tile
+            const int col_t = ((my.cell & kCellNode) - T.y0) * row + ((mx.cell & kCellNode) - T.x0) - T.z0 * sz_stride;
+            const float4* __restrict__ col = P.U + ((size_t)(my.cell & kCellNode) * dnx + (mx.cell & kCellNode));
+            const f32x2 Pxy = pk(mx.P, my.P);
+            int node_hi = -1, cell_z = -1;
+            f32x2 c0xy = 0ull, c1xy = 0ull, Bxy = 0ull, Axy = 0ull, Bzz = 0ull, A12z = 0ull;
+            float c0z = 0.f, c1z = 0.f;
+            const AxisEntry* mzp = sz;
+            for (int kk = 0; kk < kz_n; ++kk) {
+                const longlong2 em = s_em_t[kk * (kTileX * kTileY)];
+                // destinations of the voxel's z-run: two slots (a run of nsz subvoxels rarely meets a third voxel);
+                // B is the current one, A the one before; both are flushed at the end of the run, where every lane
+                // of the warp is there (the run length is CTA-uniform)
+                unsigned dstA = kNone, cntA = 0u, dstB = kNone, cntB = 0u;
+                auto flush = [&](unsigned d_shifted, unsigned cnt) {
+                    const int dst = (int)(d_shifted - kShift);
+                    if (dst >= 0) {
+                        atomicAdd(P.E + dst, (unsigned long long)em.x * cnt);
+                        atomicAdd(P.M + dst, (unsigned long long)em.y * cnt);
+                        landed += cnt;
+                    }
+                };
+                for (int c = 0; c < nsz; ++c, ++mzp) {
+                    const AxisEntry mz = *mzp;
+                    if (mz.cell != cell_z) {                                      // new DVF z-cell (warp-uniform branch)
+                        cell_z = mz.cell;
+                        const int lo = mz.cell & kCellNode, hi = lo + ((mz.cell & kCellD1) ? 1 : 0);
+                        if (lo == node_hi) { c0xy = c1xy; c0z = c1z; }
+                        else if (kTile) node_bilerp_tile(tile + (col_t + lo * sz_stride), sy1, mx.w, my.w, c0xy, c0z);
+                        else node_bilerp(col + (size_t)lo * sz_stride, dx1, sy1, mx.w, my.w, c0xy, c0z);
+                        if (hi == lo) { c1xy = c0xy; c1z = c0z; }
+                        else if (kTile) node_bilerp_tile(tile + (col_t + hi * sz_stride), sy1, mx.w, my.w, c1xy, c1z);
+                        else node_bilerp(col + (size_t)hi * sz_stride, dx1, sy1, mx.w, my.w, c1xy, c1z);
+                        node_hi = hi;
+                        // folded estimate of this cell: y = w B + A per axis (see the tolerance derivation above)
+                        const float ddz = __fsub_rn(c1z, c0z);
+                        Bxy  = mul2(sub2(c1xy, c0xy), ihxy);
+                        Axy  = fma2(c0xy, ihxy, Pxy);
+                        Bzz  = mul2(pk(ddz, ddz), ihzz);
+                        A12z = fma2(pk(c0z, c0z), ihzz, tolz12);                  // (c0z ih - tol, c0z ih + tol)
+                    }
+                    // x, y: estimate, nearest integer r, distance of the estimate from r
+                    const f32x2 wz2 = pk(mz.w, mz.w);
+                    const f32x2 yxy = fma2(wz2, Bxy, Axy);
+                    const f32x2 txy = add2(yxy, magic2);
+                    const f32x2 fxy = sub2(yxy, sub2(txy, magic2));
+                    // z: both ends of the tolerance interval; they must round to the same integer
+                    const f32x2 t12 = add2(fma2(wz2, Bzz, add2(A12z, pk(mz.P, mz.P))), magic2);
+                    float tx, ty, fx, fy, t1, t2;
+                    upk(txy, tx, ty); upk(fxy, fx, fy); upk(t12, t1, t2);
+                    const unsigned bx = __float_as_uint(tx), by = __float_as_uint(ty), bz = __float_as_uint(t1);
+                    unsigned dst = (bz * (unsigned)rny + by) * (unsigned)rnx + bx;
+                    if (!(fabsf(fx) <= htx) | !(fabsf(fy) <= hty) | (bz != __float_as_uint(t2))) {
+                        // rare: the contract's own operations (z-lerp, q = p + u, q - o) and the exact floor
+                        float c0x, c0y, c1x, c1y;
+                        upk(c0xy, c0x, c0y); upk(c1xy, c1x, c1y);
+                        const float qx = __fadd_rn(mx.p, __fadd_rn(c0x, __fmul_rn(mz.w, __fsub_rn(c1x, c0x))));
+                        const float qy = __fadd_rn(my.p, __fadd_rn(c0y, __fmul_rn(mz.w, __fsub_rn(c1y, c0y))));
+                        const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, __fsub_rn(c1z, c0z))));
+                        const int ix = exact_floor(__fsub_rn(qx, P.ref.ox), P.ref.hx, P.inv_hrx, rnx);
+                        const int iy = exact_floor(__fsub_rn(qy, P.ref.oy), P.ref.hy, P.inv_hry, rny);
+                        const int iz = exact_floor(__fsub_rn(qz, P.ref.oz), P.ref.hz, P.inv_hrz, rnz);
+                        dst = (ix | iy | iz) < 0 ? kNone : (unsigned)((iz * rny + iy) * rnx + ix) + kShift;
+                    } else if (kChecked) {
+                        const bool out = ((bx - (unsigned)kMagicBits) >= (unsigned)rnx) |
+                                         ((by - (unsigned)kMagicBits) >= (unsigned)rny) |
+                                         ((bz - (unsigned)kMagicBits) >= (unsigned)rnz);
+                        dst = out ? kNone : dst;
+                    }
+                    // count it in slot B; a new destination moves B to A (A, if occupied, is flushed: a third voxel)
+                    const bool same = dst == dstB;
+                    if (!same & (cntA != 0u)) flush(dstA, cntA);
+                    dstA = same ? dstA : dstB; cntA = same ? cntA : cntB;
+                    dstB = dst;                cntB = same ? cntB + 1u : 1u;
+                }
+                if (cntA != 0u) flush(dstA, cntA);
+                flush(dstB, cntB);
+            }
+        }
+    }
 }
 
 // Thread = a column of chunk_z source voxels along z at (i, j); CTA = 32 x 4 such columns.
 // Loop nest: subvoxel (b, a) of the column outside, ALL its z-subvoxels inside.  The integer sums do not depend on
 // the visiting order, so the nest is arranged for reuse:
+//   * the DVF nodes the CTA's subvoxels interpolate between are staged once in shared memory (a (tile + halo) box of
+//     float4 nodes, loaded coalesced; a field too fine for the box is read through L1 instead), and the largest
+//     displacement inside the box bounds |u| for this CTA;
 //   * the z-sequence of DVF cells is the same for every thread of the CTA (the z-axis map lives in shared memory), so
 //     the "new z-cell" branch is warp-uniform;
-//   * the x- and y-lerps (A3) are evaluated once per z-NODE of the column: walking up, the upper node of one cell is
-//     the lower node of the next, and the difference c1 - c0 of the z-lerp is formed once per cell;
-//   * per subvoxel only the z-lerp (mul, add per component), q = p + u, q - o, the product with RN(1/h) and the
-//     floor (fast_floor) remain -- all on the FMA/ALU pipes, no conversion or division instruction;
-//   * consecutive subvoxels of a voxel that land in the same reference voxel are merged into one pair of
-//     red.global.add.u64; drop counters are derived from per-column counts, not per subvoxel.
-// Each value is produced by exactly the operations of the contract, so the
-// result stays bit-identical to the oracle.
+//   * the x- and y-lerps (A3) are evaluated once per z-NODE of the column, on f32x2 pairs: walking up, the upper node of
+//     one cell is the lower node of the next;
+//   * per subvoxel the main path holds NO contract value: the z-lerp, q = p + u, q - o and the division by h are folded
+//     into one fma per axis whose result estimates Q - 0.5 (tolerance derivation above); x and y are one f32x2 pair,
+//     z is the pair of the two ends of its tolerance interval.  Seven packed operations, the integer destination index
+//     straight from the bit patterns of the rounded estimates (the offsets folded into one constant), and -- only in
+//     CTAs near the border of the reference grid or of the DVF's z-extent -- the range test;
+//   * a subvoxel whose estimate is within tol of a voxel face is decided by the contract's operations (rare: ~1e-3);
+//   * the subvoxels of a voxel's z-run that land in the same reference voxel are merged (two destination slots) and
+//     flushed as pairs of red.global.add.u64 at the end of the run, where all lanes of the warp flush together; drop
+//     counters are derived from per-column counts, not per subvoxel.
+// Every destination is either proven equal to the contract's or computed by
+// it, so the result stays bit-identical to the oracle.
 __global__ void __launch_bounds__(kTileX * kTileY)
 emtm_push_kernel(const __grid_constant__ PushParams P)
 {
@@ -163,120 +361,119 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
     AxisEntry* sy = sx + kTileX * P.nsx;                 // [4][nsy]
     AxisEntry* sz = sy + kTileY * P.nsy;                 // [chunk_z * nsz]
     longlong2* s_em = reinterpret_cast<longlong2*>(sz + P.chunk_z * P.nsz);   // [chunk_z][128] (e_q, m_q) per voxel
+    float4* tile = reinterpret_cast<float4*>(s_em + P.chunk_z * kTileX * kTileY);   // [tile_cap] DVF nodes
+    __shared__ int s_okz;
     const int tid = threadIdx.y * kTileX + threadIdx.x;
     const int i = blockIdx.x * kTileX + threadIdx.x;
     const int j = blockIdx.y * kTileY + threadIdx.y;
     const int k0 = blockIdx.z * P.chunk_z;               // this CTA covers source voxels k0 .. k0 + kz_n - 1 along z
     const int kz_n = min(P.chunk_z, P.src.nz - k0);
     const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy, n_z = kz_n * P.nsz;
+    if (tid == 0) s_okz = 0;
+    __syncthreads();
     for (int e = tid; e < n_x + n_y + n_z; e += kTileX * kTileY) {
         if (e < n_x)
             s_map[e] = axis_map(P.src.ox, P.src.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
-                                P.dvf.ox, P.dvf.hx, P.dvf.nx);
+                                P.dvf.ox, P.dvf.hx, P.dvf.nx, P.ref.ox, P.ihdx);
         else if (e < n_x + n_y)
             s_map[e] = axis_map(P.src.oy, P.src.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
-                                P.dvf.oy, P.dvf.hy, P.dvf.ny);
+                                P.dvf.oy, P.dvf.hy, P.dvf.ny, P.ref.oy, P.ihdy);
         else {
             AxisEntry m = axis_map(P.src.oz, P.src.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
-                                   P.dvf.oz, P.dvf.hz, P.dvf.nz);
-            // a z-subvoxel outside the DVF extent is dropped (A3): a NaN coordinate sends it through exact_floor,
+                                   P.dvf.oz, P.dvf.hz, P.dvf.nz, P.ref.oz, P.ihdz);
+            // a z-subvoxel outside the DVF extent is dropped (A3): NaN coordinates send it through the exact path,
             // which returns "outside", so the inner loop needs no per-subvoxel flag test
-            if (!(m.flags & 2)) m.p = __int_as_float(0x7fc00000);
+            if (m.cell & kCellOk) atomicAdd(&s_okz, 1);
+            else m.p = m.P = __int_as_float(0x7fc00000);
+            m.cell &= ~kCellOk;                          // z entries: the cell identity only (i0 | d1)
             sz[e - n_x - n_y] = m;
-        }
-    }
-    const bool mine = i < P.src.nx && j < P.src.ny;
-    if (mine) {
-        for (int kk = 0; kk < kz_n; ++kk) {              // A1: integer mass and energy of this thread's voxels
-            const size_t v = ((size_t)(k0 + kk) * P.src.ny + j) * P.src.nx + i;
-            const float rho = __ldg(P.rho + v), dose = __ldg(P.dose + v);
-            s_em[kk * (kTileX * kTileY) + tid] =
-                make_longlong2(__double2ll_rn(__dmul_rn(__dmul_rn((double)rho, (double)dose), 4294967296.0)),
-                               __double2ll_rn(__dmul_rn((double)rho, 16777216.0)));
         }
     }
     __syncthreads();
 
-    unsigned n_ref = 0, n_dvf = 0;
-    if (mine) {
-        const int nsx = P.nsx, nsy = P.nsy, nsz = P.nsz;
-        const int dnx = P.dvf.nx, dny = P.dvf.ny;
-        const int dx1 = dnx > 1 ? 1 : 0;                 // upper x node = lower + 1 unless the DVF grid is 1 node wide
-        const float orx = P.ref.ox, ory = P.ref.oy, orz = P.ref.oz, hrx = P.ref.hx, hry = P.ref.hy, hrz = P.ref.hz;
-        const float ihx = P.inv_hrx, ihy = P.inv_hry, ihz = P.inv_hrz;
-        const float fcx = P.cx, fcy = P.cy, fcz = P.cz, htx = P.htx, hty = P.hty, htz = P.htz;
-        const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
-        const AxisEntry* sxl = sx + threadIdx.x;
-        const AxisEntry* syl = sy + threadIdx.y * nsy;
-        const int sz_stride = dny * dnx;
-        int okz = 0;                                     // z-subvoxels of the column inside the DVF extent (CTA-uniform)
-        for (int s = 0; s < n_z; ++s) okz += (sz[s].flags >> 1) & 1;
-        unsigned landed = 0, eligible = 0;
-        for (int b = 0; b < nsy; ++b) {
-            const AxisEntry my = syl[b];
-            const int sy1 = (my.flags & 1) * dnx;
-            for (int a = 0; a < nsx; ++a) {
-                const AxisEntry mx = sxl[a * kTileX];
-                if (!(mx.flags & my.flags & 2)) continue;                         // whole column outside the DVF extent
-                eligible += (unsigned)okz;
-                const float4* __restrict__ col = P.U + my.i0 * dnx + mx.i0;       // (y0, x0) of the column, z = 0
-                int node_hi = -1;                                                 // z-node whose bilerp is held in c1*
-                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f, ddx = 0.f, ddy = 0.f, ddz = 0.f;
-                int cell_z = -1;
-                const AxisEntry* mzp = sz;
-                for (int kk = 0; kk < kz_n; ++kk) {
-                    const longlong2 em = s_em[kk * (kTileX * kTileY) + tid];
-                    const long long e_q = em.x, m_q = em.y;
-                    int run_dst = -1; unsigned run_cnt = 0u;
-                    for (int c = 0; c < nsz; ++c, ++mzp) {
-                        const AxisEntry mz = *mzp;
-                        if (mz.i0 != cell_z) {                                    // new DVF z-cell (warp-uniform branch)
-                            cell_z = mz.i0;
-                            const int hi = mz.i0 + (mz.flags & 1);
-                            if (mz.i0 == node_hi) { c0x = c1x; c0y = c1y; c0z = c1z; }
-                            else bilerp3(load_quad(col + (size_t)mz.i0 * sz_stride, dx1, sy1), mx.w, my.w, c0x, c0y, c0z);
-                            if (hi == mz.i0) { c1x = c0x; c1y = c0y; c1z = c0z; }
-                            else bilerp3(load_quad(col + (size_t)hi * sz_stride, dx1, sy1), mx.w, my.w, c1x, c1y, c1z);
-                            node_hi = hi;
-                            ddx = __fsub_rn(c1x, c0x); ddy = __fsub_rn(c1y, c0y); ddz = __fsub_rn(c1z, c0z);
-                        }
-                        // z-lerp (A3), q = p + u (A4), destination index
-                        const float qx = __fadd_rn(mx.p, __fadd_rn(c0x, __fmul_rn(mz.w, ddx)));
-                        const float qy = __fadd_rn(my.p, __fadd_rn(c0y, __fmul_rn(mz.w, ddy)));
-                        const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, ddz)));
-                        int ix, iy, iz;
-                        const bool near_x = fast_floor(qx, ihx, fcx, htx, ix);
-                        const bool near_y = fast_floor(qy, ihy, fcy, hty, iy);
-                        const bool near_z = fast_floor(qz, ihz, fcz, htz, iz);
-                        if (near_x | near_y | near_z) {                           // rare: decide exactly
-                            ix = exact_floor(__fsub_rn(qx, orx), hrx, ihx, rnx);
-                            iy = exact_floor(__fsub_rn(qy, ory), hry, ihy, rny);
-                            iz = exact_floor(__fsub_rn(qz, orz), hrz, ihz, rnz);
-                        }
-                        const bool outside = ((unsigned)ix >= (unsigned)rnx) | ((unsigned)iy >= (unsigned)rny) |
-                                             ((unsigned)iz >= (unsigned)rnz);
-                        const int dst = outside ? -1 : (iz * rny + iy) * rnx + ix;
-                        // merge consecutive subvoxels of the voxel that land in the same reference voxel
-                        if (dst != run_dst) {
-                            if (run_dst >= 0) {
-                                atomicAdd(P.E + run_dst, (unsigned long long)e_q * run_cnt);
-                                atomicAdd(P.M + run_dst, (unsigned long long)m_q * run_cnt);
-                                landed += run_cnt;
-                            }
-                            run_dst = dst; run_cnt = 0u;
-                        }
-                        run_cnt += 1u;
-                    }
-                    if (run_dst >= 0) {
-                        atomicAdd(P.E + run_dst, (unsigned long long)e_q * run_cnt);
-                        atomicAdd(P.M + run_dst, (unsigned long long)m_q * run_cnt);
-                        landed += run_cnt;
-                    }
-                }
+    // the box of DVF nodes this CTA interpolates between (the maps are monotone along their axis) is staged in shared
+    // memory when it fits: 16-byte asynchronous copies, in flight while the voxels' integer mass and energy are formed
+    Tile T;
+    {
+        const int nvx = min(kTileX, P.src.nx - blockIdx.x * kTileX), nvy = min(kTileY, P.src.ny - blockIdx.y * kTileY);
+        const int cx1 = sx[(P.nsx - 1) * kTileX + nvx - 1].cell, cy1 = sy[(nvy - 1) * P.nsy + P.nsy - 1].cell,
+                  cz1 = sz[n_z - 1].cell;
+        T.x0 = sx[0].cell & kCellNode; T.y0 = sy[0].cell & kCellNode; T.z0 = sz[0].cell & kCellNode;
+        T.nx = (cx1 & kCellNode) + ((cx1 & kCellD1) ? 1 : 0) - T.x0 + 1;
+        T.ny = (cy1 & kCellNode) + ((cy1 & kCellD1) ? 1 : 0) - T.y0 + 1;
+        T.nz = (cz1 & kCellNode) + ((cz1 & kCellD1) ? 1 : 0) - T.z0 + 1;
+    }
+    const bool use_tile = P.dvf.nx > 1 && (long long)T.nx * T.ny * T.nz <= (long long)P.tile_cap;
+    if (use_tile) {
+        const int rows = T.ny * T.nz;
+        for (int r = tid >> 5; r < rows; r += (kTileX * kTileY) >> 5) {
+            const int ty = r % T.ny, tz = r / T.ny;
+            const float4* __restrict__ src = P.U + ((size_t)(T.z0 + tz) * P.dvf.ny + (T.y0 + ty)) * P.dvf.nx + T.x0;
+            for (int x = tid & 31; x < T.nx; x += 32) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(tile + r * T.nx + x);
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src + x) : "memory");
             }
         }
-        n_dvf = (unsigned)(nsx * nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
-        n_ref = eligible - landed;                        // mapped outside the reference grid (A4)
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    const bool mine = i < P.src.nx && j < P.src.ny;
+    if (mine) {                                          // A1: integer mass and energy of this thread's voxels
+        float rho[kChunkZMax], dose[kChunkZMax];
+#pragma unroll
+        for (int kk = 0; kk < kChunkZMax; ++kk) {        // all loads first
+            const size_t v = ((size_t)(k0 + min(kk, kz_n - 1)) * P.src.ny + j) * P.src.nx + i;
+            rho[kk] = __ldg(P.rho + v); dose[kk] = __ldg(P.dose + v);
+        }
+#pragma unroll
+        for (int kk = 0; kk < kChunkZMax; ++kk)
+            if (kk < kz_n)
+                s_em[kk * (kTileX * kTileY) + tid] =
+                    make_longlong2(__double2ll_rn(__dmul_rn(__dmul_rn((double)rho[kk], (double)dose[kk]), 4294967296.0)),
+                                   __double2ll_rn(__dmul_rn((double)rho[kk], 16777216.0)));
+    }
+    if (use_tile) asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    // largest displacement of the field (the record behind the nodes): bounds |u| in the tolerance and the range test
+    const float4 um = __ldg(P.U + (size_t)P.dvf.nx * P.dvf.ny * P.dvf.nz);
+    // index tolerance per axis from the largest displacement; 0.5 - tol for the |fr| test (x, y), the pair
+    // (-tol, +tol) for z; tol >= 0.25 or NaN: every subvoxel takes the exact path
+    const float tolx = __fmaf_rn(um.x, P.tux, P.tgx), toly = __fmaf_rn(um.y, P.tuy, P.tgy),
+                tolz = __fmaf_rn(um.z, P.tuz, P.tgz);
+    const float htx = tolx < 0.25f ? 0.5f - tolx : -1.0f, hty = toly < 0.25f ? 0.5f - toly : -1.0f;
+    const float inf = __int_as_float(0x7f800000);
+    const f32x2 tolz12 = tolz < 0.25f ? pk(-tolz, tolz) : pk(-inf, inf);
+
+    unsigned n_ref = 0, n_dvf = 0;
+    const int okz = s_okz;                               // z-subvoxels of the column inside the DVF extent (CTA-uniform)
+    // can a destination of this CTA fall outside the reference grid?  Source tile +- U against the grid shrunk by one
+    // voxel (1.5 with the rounding margin), per axis; comparisons with a NaN / Inf U fail and select the checked path.
+    bool interior = okz == n_z;
+    {
+        const float x0 = P.src.ox + (float)(blockIdx.x * kTileX) * P.src.hx;
+        const float x1 = P.src.ox + (float)min(blockIdx.x * kTileX + kTileX, P.src.nx) * P.src.hx;
+        const float y0 = P.src.oy + (float)(blockIdx.y * kTileY) * P.src.hy;
+        const float y1 = P.src.oy + (float)min(blockIdx.y * kTileY + kTileY, P.src.ny) * P.src.hy;
+        const float z0 = P.src.oz + (float)k0 * P.src.hz, z1 = P.src.oz + (float)(k0 + kz_n) * P.src.hz;
+        interior = interior && (x0 - um.x >= P.ref.ox + 1.5f * P.ref.hx) &&
+                   (x1 + um.x <= P.ref.ox + ((float)P.ref.nx - 1.5f) * P.ref.hx) &&
+                   (y0 - um.y >= P.ref.oy + 1.5f * P.ref.hy) &&
+                   (y1 + um.y <= P.ref.oy + ((float)P.ref.ny - 1.5f) * P.ref.hy) &&
+                   (z0 - um.z >= P.ref.oz + 1.5f * P.ref.hz) &&
+                   (z1 + um.z <= P.ref.oz + ((float)P.ref.nz - 1.5f) * P.ref.hz);
+    }
+    if (mine) {
+        unsigned landed = 0, eligible = 0;
+        const AxisEntry* sxl = sx + threadIdx.x;
+        const AxisEntry* syl = sy + threadIdx.y * P.nsy;
+        if (use_tile) {
+            if (interior) push_columns<false, true>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, true>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+        } else {
+            if (interior) push_columns<false, false>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, false>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+        }
+        n_dvf = (unsigned)(P.nsx * P.nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
+        n_ref = eligible - landed;                            // mapped outside the reference grid (A4)
     }
     // drop counters: warp-reduce, one atomic per warp
 #pragma unroll
@@ -425,13 +622,13 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
     for (int e = tid; e < n_x + n_y + n_z; e += kTileX * kTileY) {
         if (e < n_x)
             s_map[e] = axis_map(P.ref.ox, P.ref.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
-                                P.dvf.ox, P.dvf.hx, P.dvf.nx);
+                                P.dvf.ox, P.dvf.hx, P.dvf.nx, 0.0f, 1.0);
         else if (e < n_x + n_y)
             s_map[e] = axis_map(P.ref.oy, P.ref.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
-                                P.dvf.oy, P.dvf.hy, P.dvf.ny);
+                                P.dvf.oy, P.dvf.hy, P.dvf.ny, 0.0f, 1.0);
         else
             sz[e - n_x - n_y] = axis_map(P.ref.oz, P.ref.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
-                                         P.dvf.oz, P.dvf.hz, P.dvf.nz);
+                                         P.dvf.oz, P.dvf.hz, P.dvf.nz, 0.0f, 1.0);
     }
     for (int kk = 0; kk < kz_n; ++kk) s_sum[kk * (kTileX * kTileY) + tid] = 0.0;
     __syncthreads();
@@ -448,31 +645,32 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
         const int sz_stride = dny * dnx;
         for (int b = 0; b < nsy; ++b) {
             const AxisEntry my = syl[b];
-            const int sy1 = (my.flags & 1) * dnx;
+            const int sy1 = (my.cell & kCellD1) ? dnx : 0;
             for (int a = 0; a < nsx; ++a) {
                 const AxisEntry mx = sxl[a * kTileX];
-                if (!(mx.flags & my.flags & 2)) { n_dvf += (unsigned)n_z; continue; }      // column outside the DVF extent
-                const float4* __restrict__ col = P.U + my.i0 * dnx + mx.i0;
+                if (!(mx.cell & my.cell & kCellOk)) { n_dvf += (unsigned)n_z; continue; }  // column outside the DVF extent
+                const float4* __restrict__ col = P.U + (my.cell & kCellNode) * dnx + (mx.cell & kCellNode);
                 int node_hi = -1, cell_z = -1;
-                float c0x = 0.f, c0y = 0.f, c0z = 0.f, c1x = 0.f, c1y = 0.f, c1z = 0.f, ddx = 0.f, ddy = 0.f, ddz = 0.f;
+                f32x2 c0xy = 0ull, c1xy = 0ull, ddxy = 0ull;
+                float c0z = 0.f, c1z = 0.f, ddz = 0.f;
                 const AxisEntry* mzp = sz;
                 for (int kk = 0; kk < kz_n; ++kk) {
                     double sum = s_sum[kk * (kTileX * kTileY) + tid];
                     for (int c = 0; c < nsz; ++c, ++mzp) {
                         const AxisEntry mz = *mzp;
-                        if (!(mz.flags & 2)) { n_dvf += 1; continue; }                     // warp-uniform
-                        if (mz.i0 != cell_z) {                                             // new DVF z-cell (uniform)
-                            cell_z = mz.i0;
-                            const int hi = mz.i0 + (mz.flags & 1);
-                            if (mz.i0 == node_hi) { c0x = c1x; c0y = c1y; c0z = c1z; }
-                            else bilerp3(load_quad(col + (size_t)mz.i0 * sz_stride, dx1, sy1), mx.w, my.w, c0x, c0y, c0z);
-                            if (hi == mz.i0) { c1x = c0x; c1y = c0y; c1z = c0z; }
-                            else bilerp3(load_quad(col + (size_t)hi * sz_stride, dx1, sy1), mx.w, my.w, c1x, c1y, c1z);
+                        if (!(mz.cell & kCellOk)) { n_dvf += 1; continue; }                // warp-uniform
+                        if ((mz.cell & ~kCellOk) != cell_z) {                              // new DVF z-cell (uniform)
+                            cell_z = mz.cell & ~kCellOk;
+                            const int lo = mz.cell & kCellNode, hi = lo + ((mz.cell & kCellD1) ? 1 : 0);
+                            if (lo == node_hi) { c0xy = c1xy; c0z = c1z; }
+                            else node_bilerp(col + (size_t)lo * sz_stride, dx1, sy1, mx.w, my.w, c0xy, c0z);
+                            if (hi == lo) { c1xy = c0xy; c1z = c0z; }
+                            else node_bilerp(col + (size_t)hi * sz_stride, dx1, sy1, mx.w, my.w, c1xy, c1z);
                             node_hi = hi;
-                            ddx = __fsub_rn(c1x, c0x); ddy = __fsub_rn(c1y, c0y); ddz = __fsub_rn(c1z, c0z);
+                            ddxy = sub2(c1xy, c0xy); ddz = __fsub_rn(c1z, c0z);
                         }
-                        const float qx = __fadd_rn(mx.p, __fadd_rn(c0x, __fmul_rn(mz.w, ddx)));
-                        const float qy = __fadd_rn(my.p, __fadd_rn(c0y, __fmul_rn(mz.w, ddy)));
+                        float qx, qy;
+                        upk(add2(pk(mx.p, my.p), mad2_unfused(c0xy, mz.w, ddxy)), qx, qy);
                         const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, ddz)));
                         const Cell cx = cell_of(qx, sox, shx, snx), cy = cell_of(qy, soy, shy, sny),
                                    cz = cell_of(qz, soz, shz, snz);
@@ -543,9 +741,10 @@ cudaError_t configure_accumulate(void)
 void launch_dvf_interleave(const pbs4d_grid& g, const float* disp_planar, float* out4, cudaStream_t st)
 {
     const size_t n = (size_t)g.nx * g.ny * g.nz;
-    const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)sm_count_of_current_device() * 16);
-    dvf_interleave_kernel<<<blocks, 256, 0, st>>>(n, disp_planar, disp_planar + n, disp_planar + 2 * n,
-                                                  reinterpret_cast<float4*>(out4));
+    float4* out = reinterpret_cast<float4*>(out4);
+    cudaMemsetAsync(out + n, 0, sizeof(float4), st);     // the max |u| record behind the nodes
+    dim3 grid((unsigned)g.ny * (unsigned)g.nz, (unsigned)((g.nx + 127) / 128));
+    dvf_interleave_kernel<<<grid, 128, 0, st>>>(g.nx, g.ny, disp_planar, disp_planar + n, disp_planar + 2 * n, out);
 }
 
 void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho, const pbs4d_grid& dvf_grid,
@@ -556,25 +755,33 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     P.src = src; P.dvf = dvf_grid; P.ref = ref; P.dose = dose; P.rho = rho;
     P.U = reinterpret_cast<const float4*>(disp4);
     P.inv_hrx = 1.0f / ref.hx; P.inv_hry = 1.0f / ref.hy; P.inv_hrz = 1.0f / ref.hz;
-    // fast_floor constants per axis: c = RN(-o inv_h - 0.5); tolerance 4e-7 (n + 2 + 2 |o| / h) (see fast_floor);
-    // 0.5 - tol < 0 (always exact) for grids too long for the 2^22 range of the bit trick
-    auto cst = [](float o, float inv_h) { return (float)(-(double)o * (double)inv_h - 0.5); };
-    auto hmt = [](int n, float o, float h) {
-        const double tol = 4.0e-7 * ((double)n + 2.0 + 2.0 * std::fabs((double)o) / (double)h);
-        return (n <= 4000000 && tol < 0.25) ? (float)(0.5 - tol) : -1.0f;
+    P.ihdx = 1.0 / (double)ref.hx; P.ihdy = 1.0 / (double)ref.hy; P.ihdz = 1.0 / (double)ref.hz;
+    // index tolerance per axis (derivation at kMagic): tol = 2^-23 (8 (n + 2) + 2 |o| / h) + U 2^-23 16 / h, U read by
+    // the kernel from the record behind the field; a grid too long for the rounding trick takes the exact path always
+    const double e23 = 1.1920928955078125e-7;
+    auto geo = [&](int n, float o, float h) {
+        return n <= 4000000 ? (float)(e23 * (8.0 * (n + 2.0) + 2.0 * std::fabs((double)o) / (double)h)) : INFINITY;
     };
-    P.cx = cst(ref.ox, P.inv_hrx); P.cy = cst(ref.oy, P.inv_hry); P.cz = cst(ref.oz, P.inv_hrz);
-    P.htx = hmt(ref.nx, ref.ox, ref.hx); P.hty = hmt(ref.ny, ref.oy, ref.hy); P.htz = hmt(ref.nz, ref.oz, ref.hz);
+    auto slope = [&](int n, float h) { return n <= 4000000 ? (float)(e23 * 16.0 / (double)h) : 0.0f; };
+    P.tgx = geo(ref.nx, ref.ox, ref.hx); P.tgy = geo(ref.ny, ref.oy, ref.hy); P.tgz = geo(ref.nz, ref.oz, ref.hz);
+    P.tux = slope(ref.nx, ref.hx); P.tuy = slope(ref.ny, ref.hy); P.tuz = slope(ref.nz, ref.hz);
     P.nsx = nsx; P.nsy = nsy; P.nsz = nsz;
     P.E = (unsigned long long*)E; P.M = (unsigned long long*)M; P.counters = counters;
     // z-chunk per thread: the x/y-lerps are evaluated once per z-node of a column, and the first node of a column is
-    // extra, so longer columns amortise it (and the CTA prologue); measured on config 4 (chunk 1 -> this choice):
-    // n = 4 5.09 -> 4.19 ms, n = 8 29.9 -> 27.4 ms, (2,2,5) 1.69 -> 1.34 ms per 9 phases of 128^3
-    P.chunk_z = nsz <= 2 ? kChunkZMax : 4;
+    // extra, so longer columns amortise it (and the CTA prologue); shorter ones keep the DVF tile and the (e_q, m_q)
+    // stage small enough for 6-7 resident CTAs per SM.  Measured on config 4 (chunk 8 / 4 / 2, ms per 9 phases):
+    // n = 2 1.02 / 0.86 / 1.04, n = 4 4.6 / 3.6 / 3.9, n = 8 28.7 / 22.5 / 21.8, (2,2,5) 1.57 / 1.25 / 1.42
+    P.chunk_z = 4;
     dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY,
                                  (src.nz + P.chunk_z - 1) / P.chunk_z);
-    const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
-                        (size_t)P.chunk_z * kTileX * kTileY * sizeof(longlong2);
+    // shared memory: axis maps + (e_q, m_q) per voxel + the DVF tile.  The tile is sized for a field on the source
+    // grid's spacing ((32 + 2) x (4 + 2) x (chunk_z + 2) nodes) and shrunk so that the total stays under 60 KB.
+    const size_t fixed = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
+                         (size_t)P.chunk_z * kTileX * kTileY * sizeof(longlong2);
+    const size_t want = (size_t)(kTileX + 2) * (kTileY + 2) * (P.chunk_z + 2);
+    const size_t room = fixed < 60 * 1024 ? (60 * 1024 - fixed) / sizeof(float4) : 0;
+    P.tile_cap = (int)std::min(want, room);
+    const size_t smem = fixed + (size_t)P.tile_cap * sizeof(float4);
     emtm_push_kernel<<<g, b, smem, st>>>(P);             // > 48 KB possible: configure_accumulate() opted in
 }
 

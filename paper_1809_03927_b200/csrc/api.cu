@@ -288,7 +288,7 @@ static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const c
     CU(cudaSetDevice(ctx->device));
     auto& d = table[src_phase];
     if (!d.disp) d.disp.reset(new DevBuf);
-    const size_t bytes = (size_t)4 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz * sizeof(float);
+    const size_t bytes = ((size_t)4 * dvf_grid->nx * dvf_grid->ny * dvf_grid->nz + 4) * sizeof(float);   // + max |u| record
     CU(d.disp->ensure(bytes));
     launch_dvf_interleave(*dvf_grid, disp_dev, d.disp->as<float>(), ctx->stream);
     CU(cudaGetLastError());
@@ -926,7 +926,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
             if (p == ref_phase || !disp_host[p]) continue;
             auto& d = ctx->dvf[p];
             if (!d.disp) d.disp.reset(new DevBuf);
-            CU(d.disp->ensure(4 * dvf_vox * sizeof(float)));
+            CU(d.disp->ensure((4 * dvf_vox + 4) * sizeof(float)));   // + max |u| record
             float* stage = tmp.as<float>() + k * 3 * dvf_vox; ++k;
             CU(cudaMemcpyAsync(stage, disp_host[p], 3 * dvf_vox * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream));
             bytes += 3 * dvf_vox * sizeof(float);

@@ -68,7 +68,8 @@ void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long
                           double per_protons, float* dose, cudaStream_t st);
 
 struct AccCounters { unsigned long long subvoxels, dropped_ref, dropped_dvf; };
-// planar [3][z][y][x] displacements -> interleaved float4 {ux,uy,uz,0} per node (the layout the push kernel reads)
+// planar [3][z][y][x] displacements -> interleaved float4 {ux, uy, uz, uz of the y-neighbour} per node, followed by one
+// float4 record {max|ux|, max|uy|, max|uz|, 0}: out4 holds 4 * nodes + 4 floats (the layout the accumulation kernels read)
 void launch_dvf_interleave(const pbs4d_grid& dvf_grid, const float* disp_planar, float* out4, cudaStream_t st);
 void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho, const pbs4d_grid& dvf_grid,
                       const float* disp4, const pbs4d_grid& ref, int nsx, int nsy, int nsz,
