@@ -770,8 +770,10 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     // z-chunk per thread: the x/y-lerps are evaluated once per z-node of a column, and the first node of a column is
     // extra, so longer columns amortise it (and the CTA prologue); shorter ones keep the DVF tile and the (e_q, m_q)
     // stage small enough for 6-7 resident CTAs per SM.  Measured on config 4 (chunk 8 / 4 / 2, ms per 9 phases):
-    // n = 2 1.02 / 0.86 / 1.04, n = 4 4.6 / 3.6 / 3.9, n = 8 28.7 / 22.5 / 21.8, (2,2,5) 1.57 / 1.25 / 1.42
-    P.chunk_z = 4;
+    // n = 2 1.02 / 0.86 / 1.04, n = 4 4.6 / 3.6 / 3.9, n = 8 28.7 / 22.5 / 21.8, (2,2,5) 1.57 / 1.25 / 1.42.
+    // With two z-subvoxels per voxel the CTA prologue weighs most: there the long column without the tile (the nodes
+    // through L1) is best, 0.82 ms.
+    P.chunk_z = nsz <= 2 ? kChunkZMax : 4;
     dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY,
                                  (src.nz + P.chunk_z - 1) / P.chunk_z);
     // shared memory: axis maps + (e_q, m_q) per voxel + the DVF tile.  The tile is sized for a field on the source
@@ -780,7 +782,7 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
                          (size_t)P.chunk_z * kTileX * kTileY * sizeof(longlong2);
     const size_t want = (size_t)(kTileX + 2) * (kTileY + 2) * (P.chunk_z + 2);
     const size_t room = fixed < 60 * 1024 ? (60 * 1024 - fixed) / sizeof(float4) : 0;
-    P.tile_cap = (int)std::min(want, room);
+    P.tile_cap = nsz <= 2 ? 0 : (int)std::min(want, room);
     const size_t smem = fixed + (size_t)P.tile_cap * sizeof(float4);
     emtm_push_kernel<<<g, b, smem, st>>>(P);             // > 48 KB possible: configure_accumulate() opted in
 }

@@ -72,11 +72,14 @@ __device__ __forceinline__ void philox(const Params& P, uint32_t block, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
-// u = ((x >> 9) + 0.5) 2^-23, built without an integer->float conversion: (1 + m 2^-23) - 1 + 2^-24, all exact
+// u = ((x >> 9) + 0.5) 2^-23, built without an integer->float conversion: (1 + m 2^-23) - (1 - 2^-24).  The
+// subtrahend 0x3F7FFFFF is a float and the difference (2 m + 1) 2^-24 has 24 significant bits: one exact FADD.
+constexpr float kOneMinusEps = 0.99999994039535522461f;             // 1 - 2^-24
 __device__ __forceinline__ float u01(uint32_t x)
 {
-    return (__uint_as_float(0x3F800000u | (x >> 9)) - 1.0f) + 5.9604644775390625e-8f;
+    return __uint_as_float(0x3F800000u | (x >> 9)) - kOneMinusEps;
 }
+__device__ __forceinline__ float unit_float(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)); }   // in [1, 2)
 
 __device__ __forceinline__ float fast_sqrt(float x)
 {
@@ -126,6 +129,31 @@ __device__ __forceinline__ Lookup locate(float E)
     return L;
 }
 
+// ---- packed fp32 pairs (sm_100 f32x2: one issue slot for two operations; each half rounds as the scalar op) ----
+// The kernel is bound by instruction issue, so the (x, y) halves of position and direction and the pairs of table
+// columns that are interpolated together go through FFMA2 / FMUL2 / FADD2.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi)
+{
+    f32x2 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d;
+}
+__device__ __forceinline__ void upk(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+
 // Per-lane history state.  Position p* is voxel-local: 0 <= p <= h on each axis.
 struct Lane {
     float px, py, pz, dx, dy, dz, E, wq;      // wq = weight * 2^k (deposit -> quanta)
@@ -133,7 +161,8 @@ struct Lane {
     uint32_t g_lo, g_hi, m;
     int vox;                                   // linear voxel index of the pending deposit (< 2^31 voxels)
     long long pend;                            // quanta deposited in vox and not yet flushed
-    float dens, inv_dens;                      // dens holds 0.1 x density: t [g/cm2] = dens x s [mm]
+    float rho;                                 // density of the current voxel; 0.1 rho and 1 / rho are formed at the top
+                                               // of every step, a table lookup away from the load that produced rho
     int seg;                                   // index of the history's segment in the launch table
 };
 
@@ -288,7 +317,7 @@ transport_kernel(const __grid_constant__ Params P)
                         L.wq = S.weight_scaled; L.seg = tag;
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.pend = 0;
-                        { const float rho = __ldg(P.rho + L.vox); L.dens = 0.1f * rho; L.inv_dens = fast_rcp(rho); }
+                        L.rho = __ldg(P.rho + L.vox);
                         alive = true;
                     }
                 }
@@ -308,20 +337,28 @@ transport_kernel(const __grid_constant__ Params P)
         if (alive) {
             // ---------------- one condensed-history step (T5-T10) ----------------
             L.m += 1u;
-            const float dens = L.dens;
             const Lookup k0 = locate(L.E);
             const float4 A0 = s_tab[k0.i], B0 = s_tab[k0.i + 1];
-            const float rs = fmaf(k0.f, B0.x - A0.x, A0.x);                  // 0.2 R_w(E)
-            const float S0 = fmaf(k0.f, B0.y - A0.y, A0.y);
-            const float s_lim = fminf(kSmax, rs * L.inv_dens);
+            float rs, S0;                                                     // 0.2 R_w(E), S(E): one packed interpolation
+            {
+                const f32x2 a = pk(A0.x, A0.y);
+                upk(fma2(pk(k0.f, k0.f), sub2(pk(B0.x, B0.y), a), a), rs, S0);
+            }
+            // the density was loaded when the history entered the voxel (end of the previous iteration): its reciprocal
+            // is taken here, after the table lookup, so that the load's latency hides behind the lookup instead of
+            // stalling the warp in the voxel-change block
+            const float dens = 0.1f * L.rho;                                  // t [g/cm2] = dens x s [mm]
+            const float s_lim = fminf(kSmax, rs * fast_rcp(L.rho));
 
             // T6: nearest voxel face.  Per axis: numerator = distance to the face ahead, denominator = |d|;
             // the smallest quotient is found by cross-multiplication, then one reciprocal.
             // (direction components are never exactly zero: a zero component of the field direction is replaced by
             // +1e-20 when the history starts, which keeps that axis' quotient astronomically large, as 1/0 would)
             const float denx = fabsf(L.dx), deny = fabsf(L.dy), denz = fabsf(L.dz);
-            const float numx = fmaxf(L.dx > 0.0f ? hx - L.px : L.px, 0.0f);
-            const float numy = fmaxf(L.dy > 0.0f ? hy - L.py : L.py, 0.0f);
+            float hpx, hpy;
+            upk(sub2(pk(hx, hy), pk(L.px, L.py)), hpx, hpy);
+            const float numx = fmaxf(L.dx > 0.0f ? hpx : L.px, 0.0f);
+            const float numy = fmaxf(L.dy > 0.0f ? hpy : L.py, 0.0f);
             const float numz = fmaxf(L.dz > 0.0f ? hz - L.pz : L.pz, 0.0f);
             // x against z, then y against the winner; equal cross products mark axes that attain the minimum together
             const float cxz = numx * denz, czx = numz * denx;
@@ -356,11 +393,20 @@ transport_kernel(const __grid_constant__ Params P)
             // T8: straggling (Philox block m): sigma g = sqrt(V t (-2 ln u2)) cos(2 pi u3)
             uint32_t r0, r1, r2, r3;
             philox(P, L.m, L.g_lo, L.g_hi, r0, r1, r2, r3);
+            // Bohr variance and theta0^2 at E_m (one packed interpolation), both uniforms of the Gaussian magnitudes
+            // (one packed subtraction), and the two products -V t lg u2, -T t lg u0 (two packed multiplications)
+            float varg, th2;
+            {
+                const f32x2 a  = pk(Am.z, Am.w);
+                const f32x2 vt = fma2(pk(fm, fm), sub2(pk(Bm.z, Bm.w), a), a);                       // (V, T)
+                float u2, u0;
+                upk(sub2(pk(unit_float(r2), unit_float(r0)), pk(kOneMinusEps, kOneMinusEps)), u2, u0);
+                upk(mul2(mul2(vt, pk(-t, -t)), pk(fast_log2(u2), fast_log2(u0))), varg, th2);
+            }
             float dE = dEm;
             if (kStrag) {
-                const float V2 = fmaf(fm, Bm.z - Am.z, Am.z);
                 const float a3 = angle_from_word(r3);
-                dE = fmaf(fast_sqrt(-V2 * t * fast_log2(u01(r2))), -__cosf(a3), dEm);
+                dE = fmaf(fast_sqrt(varg), -__cosf(a3), dEm);
             }
             dE = fminf(fmaxf(dE, 0.0f), L.E);
             if (L.E - dE <= kEcut) { dE = L.E; alive = false; }
@@ -368,7 +414,8 @@ transport_kernel(const __grid_constant__ Params P)
             // T9/T11: score into the voxel the step lay in (register accumulation, flushed on voxel change)
             L.pend += __float2ll_rn(dE * L.wq);
 
-            L.px = fmaf(s, L.dx, L.px); L.py = fmaf(s, L.dy, L.py); L.pz = fmaf(s, L.dz, L.pz);
+            upk(fma2(pk(s, s), pk(L.dx, L.dy), pk(L.px, L.py)), L.px, L.py);
+            L.pz = fmaf(s, L.dz, L.pz);
 
             // T10: boundary-limited step -> snap every axis attaining the minimum onto its face (branch-free)
             mx = mx && crossing; my = my && crossing; mz = mz && crossing;
@@ -378,28 +425,39 @@ transport_kernel(const __grid_constant__ Params P)
                 L.iy += my ? (fy ? 1 : -1) : 0; L.py = my ? (fy ? 0.0f : hy) : L.py;
                 L.iz += mz ? (fz ? 1 : -1) : 0; L.pz = mz ? (fz ? 0.0f : hz) : L.pz;
             }
-
             // T9: Highland deflection at the end of the step (kinematics at Em), branch-free orthonormal basis;
             // theta^2 = T t (-2 ln u0); sin and cos of the (small) polar angle by their Taylor polynomials
             if (kMcs) {
-                const float T2  = fmaf(fm, Bm.w - Am.w, Am.w);
-                const float th2 = -T2 * t * fast_log2(u01(r0));
                 const float th  = fast_sqrt(th2);
-                const float st  = th * fmaf(th2, fmaf(th2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
-                const float ct  = fmaf(th2, fmaf(th2, fmaf(th2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
+                // sin(th) / th = 1 + th2 (-1/6 + th2 / 120) and cos(th) = 1 + th2 (-1/2 + th2 (1/24 - th2 / 720)): the two
+                // Horner chains advance together, two packed fmas
+                float ps, pc;
+                {
+                    const f32x2 t2 = pk(th2, th2);
+                    const f32x2 h1 = fma2(t2, pk(1.0f / 120.0f, -1.0f / 720.0f), pk(-1.0f / 6.0f, 1.0f / 24.0f));
+                    upk(fma2(t2, h1, pk(1.0f, -0.5f)), ps, pc);
+                }
+                const float st  = th * ps;
+                const float ct  = fmaf(th2, pc, 1.0f);
                 float sp, cp;
                 const float a1 = angle_from_word(r1);
                 sp = -__sinf(a1); cp = -__cosf(a1);
                 const float sw = copysignf(1.0f, L.dz);
                 const float aa = -fast_rcp(sw + L.dz);
                 const float bb = L.dx * L.dy * aa;
-                const float e1x = fmaf(sw * L.dx, L.dx * aa, 1.0f), e1y = sw * bb, e1z = -sw * L.dx;
-                const float e2x = bb, e2y = fmaf(L.dy, L.dy * aa, sw), e2z = -L.dy;
-                const float ux = fmaf(cp, e1x, sp * e2x), uy = fmaf(cp, e1y, sp * e2y), uz = fmaf(cp, e1z, sp * e2z);
-                const float nxd = fmaf(ct, L.dx, st * ux), nyd = fmaf(ct, L.dy, st * uy), nzd = fmaf(ct, L.dz, st * uz);
+                float dxa, dya;
+                upk(mul2(pk(L.dx, L.dy), pk(aa, aa)), dxa, dya);
+                const float e1x = fmaf(sw * L.dx, dxa, 1.0f), e1y = sw * bb, e1z = -sw * L.dx;
+                const float e2x = bb, e2y = fmaf(L.dy, dya, sw), e2z = -L.dy;
+                const f32x2 uxy = fma2(pk(cp, cp), pk(e1x, e1y), mul2(pk(sp, sp), pk(e2x, e2y)));
+                const float uz  = fmaf(cp, e1z, sp * e2z);
+                const f32x2 nxy = fma2(pk(ct, ct), pk(L.dx, L.dy), mul2(pk(st, st), uxy));
+                const float nzd = fmaf(ct, L.dz, st * uz);
+                float nxd, nyd;
+                upk(nxy, nxd, nyd);
                 const float n2  = fmaf(nxd, nxd, fmaf(nyd, nyd, nzd * nzd));
                 const float inv = fmaf(-0.5f, n2, 1.5f);                      // 1/sqrt(n2) to first order, n2 = 1 + O(1e-6)
-                L.dx = nxd * inv; L.dy = nyd * inv; L.dz = nzd * inv;
+                upk(mul2(nxy, pk(inv, inv)), L.dx, L.dy); L.dz = nzd * inv;
             }
             L.E -= dE;
 
@@ -413,8 +471,8 @@ transport_kernel(const __grid_constant__ Params P)
                         alive = false;
                         n_steps += L.m;
                     } else {
-                        L.vox  = (L.iz * ny + L.iy) * nx + L.ix;
-                        { const float rho = __ldg(P.rho + L.vox); L.dens = 0.1f * rho; L.inv_dens = fast_rcp(rho); }
+                        L.vox = (L.iz * ny + L.iy) * nx + L.ix;
+                        L.rho = __ldg(P.rho + L.vox);
                     }
                 }
             }
