@@ -225,14 +225,14 @@ struct Tile { int x0, y0, z0, nx, ny, nz; };
 // kChecked = false: the CTA's source tile, displaced by at most U, lies at least one voxel inside the reference grid
 // on every axis and entirely inside the DVF grid's z-extent, so no destination can fall outside and the range test is
 // compiled out.  kTile: the DVF nodes come from the CTA's shared-memory tile instead of global memory.
-template <bool kChecked, bool kTile>
+template <bool kChecked, bool kTile, int kNsz>
 __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntry* __restrict__ sxl,
                                              const AxisEntry* __restrict__ syl, const AxisEntry* __restrict__ sz,
                                              const longlong2* __restrict__ s_em_t, const float4* tile, const Tile T,
                                              int kz_n, int okz, float htx, float hty, f32x2 tolz12, unsigned& eligible,
                                              unsigned& landed)
 {
-    const int nsx = P.nsx, nsy = P.nsy, nsz = P.nsz;
+    const int nsx = P.nsx, nsy = P.nsy, nsz = kNsz ? kNsz : P.nsz;      // kNsz > 0: the z-run is unrolled
     const int dnx = P.dvf.nx;
     const int dx1 = dnx > 1 ? 1 : 0;                     // upper x node = lower + 1 unless the DVF grid is 1 node wide
     const int rnx = P.ref.nx, rny = P.ref.ny, rnz = P.ref.nz;
@@ -272,6 +272,7 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
                         landed += cnt;
                     }
                 };
+#pragma unroll
                 for (int c = 0; c < nsz; ++c, ++mzp) {
                     const AxisEntry mz = *mzp;
                     if (mz.cell != cell_z) {                                      // new DVF z-cell (warp-uniform branch)
@@ -353,6 +354,7 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
 //     counters are derived from per-column counts, not per subvoxel.
 // Every destination is either proven equal to the contract's or computed by
 // it, so the result stays bit-identical to the oracle.
+template <int kNsz>
 __global__ void __launch_bounds__(kTileX * kTileY)
 emtm_push_kernel(const __grid_constant__ PushParams P)
 {
@@ -466,11 +468,11 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * P.nsy;
         if (use_tile) {
-            if (interior) push_columns<false, true>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, true>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, true, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, true, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
         } else {
-            if (interior) push_columns<false, false>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, false>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, false, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, false, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
         }
         n_dvf = (unsigned)(P.nsx * P.nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
         n_ref = eligible - landed;                            // mapped outside the reference grid (A4)
@@ -733,7 +735,9 @@ cudaError_t configure_accumulate(void)
 {
     // the push kernel's axis maps + per-voxel (e_q, m_q) stage need up to 57 KB of dynamic shared memory at 64
     // subvoxels per axis.  A per-device attribute: pbs4d_create calls this for every context.
-    cudaError_t e = cudaFuncSetAttribute(emtm_push_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaError_t e = cudaSuccess;
+    for (void (*k)(const PushParams) : { emtm_push_kernel<0>, emtm_push_kernel<2> })
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(dim_pull_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     return e;
 }
@@ -784,7 +788,11 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     const size_t room = fixed < 60 * 1024 ? (60 * 1024 - fixed) / sizeof(float4) : 0;
     P.tile_cap = nsz <= 2 ? 0 : (int)std::min(want, room);
     const size_t smem = fixed + (size_t)P.tile_cap * sizeof(float4);
-    emtm_push_kernel<<<g, b, smem, st>>>(P);             // > 48 KB possible: configure_accumulate() opted in
+    // the two-subvoxel z-run of nsz = 2 is unrolled (config 4, 9 phases: 0.82 -> 0.73 ms); longer runs are not: the
+    // unrolled body repeats the cell-change block and outgrows the instruction cache (nsz = 8: 22.5 -> 38 ms, nsz = 5:
+    // 1.25 -> 1.63 ms).  (> 48 KB of shared memory possible: configure_accumulate() opted in)
+    void (*kernel)(const PushParams) = nsz == 2 ? emtm_push_kernel<2> : emtm_push_kernel<0>;
+    kernel<<<g, b, smem, st>>>(P);
 }
 
 void launch_emtm_finalize(const pbs4d_grid& ref, const float* dose_ref, int n_src, const long long* const* E_host,
