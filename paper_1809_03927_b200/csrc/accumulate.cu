@@ -829,7 +829,9 @@ void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs
     PullParams P;
     P.ref = ref; P.dvf = dvf_grid; P.src = src; P.U = reinterpret_cast<const float4*>(disp4); P.dose = dose_src;
     P.acc = acc; P.nsx = nsx; P.nsy = nsy; P.nsz = nsz; P.counters = counters;
-    P.chunk_z = nsz <= 2 ? kChunkZMax : 4;               // as for the push: longer columns amortise the first z-node
+    // as for the push, longer columns amortise the first z-node and the CTA prologue; measured on config 4 (ms per 9
+    // phases, chunk 4 / 8 / 16 / 32): n = 1 0.395 / 0.358 / 0.336 / 0.573, n = 2 1.45 / 1.43 / 1.42 / 2.26
+    P.chunk_z = nsz <= 2 ? 16 : 4;
     dim3 b(kTileX, kTileY, 1), g((ref.nx + kTileX - 1) / kTileX, (ref.ny + kTileY - 1) / kTileY,
                                  (ref.nz + P.chunk_z - 1) / P.chunk_z);
     const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
