@@ -67,15 +67,17 @@ def test_config4_small_bit_exact(ctx, ns):
     assert_bit_exact(gpu_accumulate(ctx, c, ns), oracle_accumulate(c, ns))
 
 
-def test_coarse_and_partial_dvf_grid(ctx):
+@pytest.mark.parametrize("ns", [(2, 2, 2), (3, 4, 4)])
+def test_coarse_and_partial_dvf_grid(ctx, ns):
     # DVF on a coarser grid (paper Table I: deformation grids ~2x coarser than the CT) that does not cover the dose
-    # grid: exercises clamp-to-edge, the outside-DVF drop and the coverage mask
+    # grid: exercises clamp-to-edge, the outside-DVF drop and the coverage mask; nsz = 4 also the shared-memory node
+    # box with z-subvoxels outside the DVF extent
     c = synth.config4(n=40, n_phases=3, dvf_div=2)
     dg = c["dvf_grid"].copy()
     dg["ox"], dg["oy"], dg["oz"] = 6.0, 3.0, 9.0
     grids = [dg, dg, dg]
-    g = gpu_accumulate(ctx, c, (2, 2, 2), dvf_grids=grids)
-    o = oracle_accumulate(c, (2, 2, 2), dvf_grids=grids)
+    g = gpu_accumulate(ctx, c, ns, dvf_grids=grids)
+    o = oracle_accumulate(c, ns, dvf_grids=grids)
     assert_bit_exact(g, o)
     assert g[1]["dropped_outside_dvf"] > 0 and g[1]["dropped_outside_ref"] > 0
     assert (g[0] == 0).any() and (g[0] != 0).any()
@@ -90,6 +92,51 @@ def test_anisotropic_voxels(ctx):
     for p in range(1, 3):
         c["disps"][p] = (c["disps"][p] * 0.3).astype(np.float32)
     assert_bit_exact(gpu_accumulate(ctx, c, (2, 2, 5)), oracle_accumulate(c, (2, 2, 5)))
+
+
+def test_huge_displacements_take_the_exact_path(ctx):
+    # |u| of thousands of voxels: the index tolerance exceeds 1/4 and every subvoxel is decided by the contract's own
+    # operations (the estimate is never trusted); nearly everything lands outside the reference grid
+    c = synth.config4(n=24, n_phases=3)
+    for p in range(1, 3):
+        c["disps"][p] = (c["disps"][p] * np.float32(3.0e5)).astype(np.float32)
+        c["disps"][p][:, ::3, ::2, ::2] *= np.float32(1.0e-5)            # some nodes stay small: a few subvoxels land
+    g = gpu_accumulate(ctx, c, (2, 2, 2)); o = oracle_accumulate(c, (2, 2, 2))
+    assert_bit_exact(g, o)
+    assert g[1]["dropped_outside_ref"] > 0.5 * g[1]["subvoxels"]
+    assert_bit_exact(gpu_accumulate(ctx, c, (3, 3, 4)), oracle_accumulate(c, (3, 3, 4)))
+
+
+def test_non_finite_nodes_are_dropped_like_the_oracle_drops_them(ctx):
+    # NaN / Inf displacements: the max |u| record is not finite, so the kernel takes the exact path everywhere and the
+    # subvoxels that interpolate a bad node fall outside, exactly as floorf() of a NaN does in the oracle
+    c = synth.config4(n=28, n_phases=3)
+    c["disps"][1][0, 5:8, 9:12, 3:6] = np.nan
+    c["disps"][1][2, 15, 15, 15] = np.inf
+    c["disps"][2][1, 20:22, 4, 7] = -np.inf
+    for ns in [(2, 2, 2), (4, 4, 4)]:
+        g = gpu_accumulate(ctx, c, ns); o = oracle_accumulate(c, ns)
+        assert_bit_exact(g, o)
+        assert g[1]["dropped_outside_ref"] > 0
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_dvf_grid_one_node_wide(ctx, axis):
+    # a DVF grid with a single node along one axis (upper node = lower node on that axis; the node box in shared
+    # memory is not used when the grid is one node wide in x)
+    c = synth.config4(n=32, n_phases=3)
+    name = "xyz"[axis]
+    dg = c["dvf_grid"].copy()
+    n_ax = int(dg["n" + name][0]) if hasattr(dg["n" + name], "__len__") else int(dg["n" + name])
+    dg["h" + name] = dg["h" + name] * n_ax
+    dg["n" + name] = 1
+    for p in range(1, 3):
+        sl = [slice(None)] * 4
+        sl[3 - axis] = slice(n_ax // 2, n_ax // 2 + 1)                  # disps: [3][z][y][x]
+        c["disps"][p] = np.ascontiguousarray(c["disps"][p][tuple(sl)])
+    grids = [dg, dg, dg]
+    for ns in [(2, 2, 2), (3, 3, 4)]:
+        assert_bit_exact(gpu_accumulate(ctx, c, ns, dvf_grids=grids), oracle_accumulate(c, ns, dvf_grids=grids))
 
 
 def test_identity_dvf_is_the_plain_sum(ctx):
