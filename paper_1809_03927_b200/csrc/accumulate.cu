@@ -18,6 +18,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstring>
 
 namespace pbs4d {
 
@@ -582,22 +583,42 @@ struct PullParams {
     double* acc;                             // [ref voxels]
     int nsx, nsy, nsz;
     int chunk_z;                             // reference voxels along z handled by one thread
+    float inv_shx, inv_shy, inv_shz;         // RN(1 / h) of the source grid (div_by_known)
     AccCounters* counters;
 };
 
-struct Cell { int i0, d1; float w; bool ok; };
-__device__ __forceinline__ Cell cell_of(float p, float o, float h, int n)
+// source-grid cell of a coordinate (D2): lower node i0 in [0, max(n - 2, 0)], weight w, inside flag.  The upper node is
+// i0 + 1 for every cell of a grid with n >= 2 nodes (i0 <= n - 2) and i0 itself when n == 1: a per-axis constant.
+struct Cell { int i0; float w; bool ok; };
+__device__ __forceinline__ Cell cell_from_quotient(float Q, int n)      // Q = RN(RN(p - o) / h)
 {
     Cell c;
-    float g = __fsub_rn(__fdiv_rn(__fsub_rn(p, o), h), 0.5f);
+    float g = __fsub_rn(Q, 0.5f);
     c.ok = (g >= -0.5f) && (g < __fsub_rn((float)n, 0.5f));
     g = fminf(fmaxf(g, 0.0f), (float)(n - 1));
-    int k = (int)floorf(g);
-    k = max(min(k, n - 2), 0);
+    const int k = max(min(__float2int_rd(g), n - 2), 0);
     c.i0 = k;
-    c.d1 = min(k + 1, n - 1) - k;
     c.w  = __fsub_rn(g, (float)k);
     return c;
+}
+// The correctly rounded quotient RN(e / h) without the division sequence, for a divisor whose reciprocal is at hand
+// (Markstein's correction): y = RN(1 / h), q0 = RN(e y), r = e - h q0 (exact, one fma), q1 = RN(q0 + r y) = RN(e / h) for
+// every e, provided the significand of h is not all ones and nothing underflows.  The launcher tests the proviso and
+// falls back to __fdiv_rn (kFastDiv = false); tests/test_markstein_division.py checks the identity exhaustively over all
+// 2^23 significands of e for the spacings of the configs and for random ones.  These are true fused operations by
+// design (they are not part of the contract's rounding sequence: only their RESULT, the IEEE quotient, is).
+__device__ __forceinline__ float div_by_known(float e, float h, float inv_h)
+{
+    const float q0 = __fmul_rn(e, inv_h);
+    return __fmaf_rn(__fmaf_rn(-h, q0, e), inv_h, q0);
+}
+__device__ __forceinline__ f32x2 div2_by_known(f32x2 e, f32x2 neg_h, f32x2 inv_h)
+{
+    f32x2 q0, r, q1;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(q0) : "l"(e), "l"(inv_h));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(neg_h), "l"(q0), "l"(e));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(q1) : "l"(r), "l"(inv_h), "l"(q0));
+    return q1;
 }
 
 // Thread = a column of chunk_z reference voxels at (i, j); CTA = 32 x 4 columns.  Loop nest as in the push: subvoxel
@@ -605,8 +626,10 @@ __device__ __forceinline__ Cell cell_of(float p, float o, float h, int n)
 // evaluated once per z-NODE (the upper node of a cell is the lower node of the next) and the "new z-cell" branch is
 // warp-uniform.  The double sum of a voxel receives its values in (b, a, c) order -- reading D4 -- because every voxel
 // of the column keeps its own running sum (shared memory) and the c-run of a (b, a) column is added to it value by
-// value.  Per subvoxel: z-lerp, q = r + u, the source-grid cell of q (three IEEE divisions: the continuous index is
-// needed as a value, not only its floor), 8 dose loads, 7 lerps, one double add.
+// value.  Per subvoxel: z-lerp, q = r + u, the source-grid cell of q (three IEEE quotients -- the continuous index is
+// needed as a value, not only its floor -- by Markstein's correction with the known reciprocal of the spacing), 8 dose loads, 7 lerps (the six in x and y as f32x2 pairs), one double add.
+// kX1 = 1: the source grid has more than one node along x (0: a single one); kFastDiv: see div_by_known
+template <int kX1, bool kFastDiv>
 __global__ void __launch_bounds__(kTileX * kTileY)
 dim_pull_kernel(const __grid_constant__ PullParams P)
 {
@@ -641,6 +664,8 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
         const int dnx = P.dvf.nx, dny = P.dvf.ny;
         const int dx1 = dnx > 1 ? 1 : 0;
         const int snx = P.src.nx, sny = P.src.ny, snz = P.src.nz;
+        const int row = sny > 1 ? snx : 0;                                   // offset of the upper y / z node (D2)
+        const size_t plane = snz > 1 ? (size_t)sny * snx : 0;
         const float sox = P.src.ox, soy = P.src.oy, soz = P.src.oz, shx = P.src.hx, shy = P.src.hy, shz = P.src.hz;
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * nsy;
@@ -674,18 +699,31 @@ dim_pull_kernel(const __grid_constant__ PullParams P)
                         float qx, qy;
                         upk(add2(pk(mx.p, my.p), mad2_unfused(c0xy, mz.w, ddxy)), qx, qy);
                         const float qz = __fadd_rn(mz.p, __fadd_rn(c0z, __fmul_rn(mz.w, ddz)));
-                        const Cell cx = cell_of(qx, sox, shx, snx), cy = cell_of(qy, soy, shy, sny),
-                                   cz = cell_of(qz, soz, shz, snz);
+                        // continuous source-grid index per axis: three IEEE quotients (D2)
+                        float Qx, Qy, Qz;
+                        if (kFastDiv) {
+                            upk(div2_by_known(sub2(pk(qx, qy), pk(sox, soy)), pk(-shx, -shy), pk(P.inv_shx, P.inv_shy)), Qx, Qy);
+                            Qz = div_by_known(__fsub_rn(qz, soz), shz, P.inv_shz);
+                        } else {
+                            Qx = __fdiv_rn(__fsub_rn(qx, sox), shx); Qy = __fdiv_rn(__fsub_rn(qy, soy), shy);
+                            Qz = __fdiv_rn(__fsub_rn(qz, soz), shz);
+                        }
+                        const Cell cx = cell_from_quotient(Qx, snx), cy = cell_from_quotient(Qy, sny),
+                                   cz = cell_from_quotient(Qz, snz);
                         if (!(cx.ok && cy.ok && cz.ok)) { n_src += 1; continue; }
+                        // 8 dose nodes: one 64-bit address, the x-neighbour at a compile-time offset (kX1), the y- and
+                        // z-neighbours at CTA-uniform offsets; the four x-lerps and the two y-lerps as f32x2 pairs
                         const float* __restrict__ d00 = P.dose + ((size_t)cz.i0 * sny + cy.i0) * snx + cx.i0;
-                        const float* __restrict__ d01 = d00 + cy.d1 * snx;
-                        const float* __restrict__ d10 = d00 + (size_t)cz.d1 * sny * snx;
-                        const float* __restrict__ d11 = d10 + cy.d1 * snx;
-                        const float c00 = lerp_rn(__ldg(d00), __ldg(d00 + cx.d1), cx.w);
-                        const float c01 = lerp_rn(__ldg(d01), __ldg(d01 + cx.d1), cx.w);
-                        const float c10 = lerp_rn(__ldg(d10), __ldg(d10 + cx.d1), cx.w);
-                        const float c11 = lerp_rn(__ldg(d11), __ldg(d11 + cx.d1), cx.w);
-                        const float val = lerp_rn(lerp_rn(c00, c01, cy.w), lerp_rn(c10, c11, cy.w), cz.w);
+                        const float* __restrict__ d01 = d00 + row;
+                        const float* __restrict__ d10 = d00 + plane;
+                        const float* __restrict__ d11 = d10 + row;
+                        const f32x2 cy0 = lerp2(pk(__ldg(d00), __ldg(d01)), pk(__ldg(d00 + kX1), __ldg(d01 + kX1)), cx.w);
+                        const f32x2 cy1 = lerp2(pk(__ldg(d10), __ldg(d11)), pk(__ldg(d10 + kX1), __ldg(d11 + kX1)), cx.w);
+                        float c00, c01, c10, c11;
+                        upk(cy0, c00, c01); upk(cy1, c10, c11);
+                        float v0, v1;
+                        upk(lerp2(pk(c00, c10), pk(c01, c11), cy.w), v0, v1);
+                        const float val = lerp_rn(v0, v1, cz.w);
                         sum = __dadd_rn(sum, (double)val);
                     }
                     s_sum[kk * (kTileX * kTileY) + tid] = sum;
@@ -738,7 +776,9 @@ cudaError_t configure_accumulate(void)
     cudaError_t e = cudaSuccess;
     for (void (*k)(const PushParams) : { emtm_push_kernel<0>, emtm_push_kernel<2> })
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(dim_pull_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    for (void (*k)(const PullParams) : { dim_pull_kernel<0, false>, dim_pull_kernel<0, true>, dim_pull_kernel<1, false>,
+                                         dim_pull_kernel<1, true> })
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     return e;
 }
 
@@ -836,7 +876,16 @@ void launch_dim_pull(const pbs4d_grid& ref, int nsx, int nsy, int nsz, const pbs
                                  (ref.nz + P.chunk_z - 1) / P.chunk_z);
     const size_t smem = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
                         (size_t)P.chunk_z * kTileX * kTileY * sizeof(double);
-    dim_pull_kernel<<<g, b, smem, st>>>(P);              // <= 52 KB: configure_accumulate() opted in
+    // Markstein's division needs a spacing whose significand is not all ones (and a normal, finite one)
+    auto known_ok = [](float h) {
+        uint32_t b; std::memcpy(&b, &h, 4);
+        return std::isfinite(h) && h >= 1.0e-30f && h <= 1.0e30f && (b & 0x7FFFFFu) != 0x7FFFFFu;
+    };
+    P.inv_shx = 1.0f / src.hx; P.inv_shy = 1.0f / src.hy; P.inv_shz = 1.0f / src.hz;
+    const bool fast = known_ok(src.hx) && known_ok(src.hy) && known_ok(src.hz);
+    void (*kernel)(const PullParams) = src.nx > 1 ? (fast ? dim_pull_kernel<1, true> : dim_pull_kernel<1, false>)
+                                                  : (fast ? dim_pull_kernel<0, true> : dim_pull_kernel<0, false>);
+    kernel<<<g, b, smem, st>>>(P);                         // <= 60 KB: configure_accumulate() opted in
 }
 
 void launch_dim_final(const pbs4d_grid& ref, int n_src, const pbs4d_grid* dvf_grids_host, const double* acc,

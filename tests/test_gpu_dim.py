@@ -69,6 +69,27 @@ def test_coarse_partial_dvf_grid_and_anisotropic_voxels(ctx):
     assert_bit_exact(gpu_dim(ctx, c, (2, 2, 5)), oracle_dim(c, (2, 2, 5)))
 
 
+def test_spacings_that_exclude_the_known_reciprocal_division(ctx):
+    # a spacing whose significand is all ones (0x3FFFFFFF, just below 2 mm) is the exception of Markstein's correction:
+    # the launcher must fall back to the IEEE division; a neighbouring spacing takes the fast path.  Also a source grid
+    # of a single node along x (the x-neighbour of a dose node is the node itself).
+    for hx in (np.nextafter(np.float32(2.0), np.float32(0.0)), np.nextafter(np.float32(2.0), np.float32(3.0))):
+        c = synth.config4(n=30, n_phases=3)
+        for name in ("grid", "dvf_grid"):
+            c[name] = c[name].copy()
+            c[name]["hx"] = hx; c[name]["hz"] = 1.27
+        assert_bit_exact(gpu_dim(ctx, c, (2, 2, 3)), oracle_dim(c, (2, 2, 3)))
+    c = synth.config4(n=24, n_phases=3)
+    for name in ("grid", "dvf_grid"):
+        c[name] = c[name].copy()
+        c[name]["nx"] = 1
+    c["doses"] = np.ascontiguousarray(c["doses"][:, :, :, 11:12]); c["rhos"] = np.ascontiguousarray(c["rhos"][:, :, :, 11:12])
+    for p in range(1, 3):
+        c["disps"][p] = np.ascontiguousarray(c["disps"][p][:, :, :, 11:12])
+        c["disps"][p][0] *= 0.02                                           # keep the images inside the single x-voxel
+    assert_bit_exact(gpu_dim(ctx, c, (2, 2, 2)), oracle_dim(c, (2, 2, 2)))
+
+
 def test_identity_field_is_the_plain_sum(ctx):
     # "the same CT image for all phases ... identity" must reproduce the static sum
     c = synth.config4(n=33, n_phases=3)
