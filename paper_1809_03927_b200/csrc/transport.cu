@@ -154,6 +154,15 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
     f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
 }
 
+// one table node from shared memory at a 32-bit shared address (the compiler otherwise rebuilds the generic address of
+// the table -- S2R SR_CgaCtaId, MOV, LEA -- in every iteration of the step loop)
+__device__ __forceinline__ float4 lds_node(unsigned addr)
+{
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 // Per-lane history state.  Position p* is voxel-local: 0 <= p <= h on each axis.
 struct Lane {
     float px, py, pz, dx, dy, dz, E, wq;      // wq = weight * 2^k (deposit -> quanta)
@@ -253,6 +262,8 @@ transport_kernel(const __grid_constant__ Params P)
     __shared__ long long s_tally[6];
     __shared__ uint32_t s_pool[kWarps][kPoolWords][32];
     for (int i = threadIdx.x; i < kTabNodes; i += kThreads) s_tab[i] = P.tab[i];
+    unsigned tab_addr;                                  // laundered through asm: kept in a register, not rebuilt per step
+    asm volatile("mov.u32 %0, %1;" : "=r"(tab_addr) : "r"((unsigned)__cvta_generic_to_shared(s_tab)));
     if (threadIdx.x < 6) s_tally[threadIdx.x] = 0;
     __syncthreads();
 
@@ -338,7 +349,7 @@ transport_kernel(const __grid_constant__ Params P)
             // ---------------- one condensed-history step (T5-T10) ----------------
             L.m += 1u;
             const Lookup k0 = locate(L.E);
-            const float4 A0 = s_tab[k0.i], B0 = s_tab[k0.i + 1];
+            const float4 A0 = lds_node(tab_addr + (unsigned)k0.i * 16u), B0 = lds_node(tab_addr + (unsigned)k0.i * 16u + 16u);
             float rs, S0;                                                     // 0.2 R_w(E), S(E): one packed interpolation
             {
                 const f32x2 a = pk(A0.x, A0.y);
@@ -385,7 +396,7 @@ transport_kernel(const __grid_constant__ Params P)
             float4 Am = A0, Bm = B0;
             if (k0.f - fm > 4.0f) {
                 const Lookup km = locate(L.E - half);
-                Am = s_tab[km.i]; Bm = s_tab[km.i + 1]; fm = km.f;
+                Am = lds_node(tab_addr + (unsigned)km.i * 16u); Bm = lds_node(tab_addr + (unsigned)km.i * 16u + 16u); fm = km.f;
             }
             const float Sm  = fmaf(fm, Bm.y - Am.y, Am.y);
             const float dEm = Sm * t;
