@@ -226,7 +226,7 @@ struct Tile { int x0, y0, z0, nx, ny, nz; };
 // kChecked = false: the CTA's source tile, displaced by at most U, lies at least one voxel inside the reference grid
 // on every axis and entirely inside the DVF grid's z-extent, so no destination can fall outside and the range test is
 // compiled out.  kTile: the DVF nodes come from the CTA's shared-memory tile instead of global memory.
-template <bool kChecked, bool kTile, int kNsz>
+template <bool kChecked, bool kTile, int kNsz, int kTY>
 __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntry* __restrict__ sxl,
                                              const AxisEntry* __restrict__ syl, const AxisEntry* __restrict__ sz,
                                              const longlong2* __restrict__ s_em_t, const float4* tile, const Tile T,
@@ -260,7 +260,7 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
             float c0z = 0.f, c1z = 0.f;
             const AxisEntry* mzp = sz;
             for (int kk = 0; kk < kz_n; ++kk) {
-                const longlong2 em = s_em_t[kk * (kTileX * kTileY)];
+                const longlong2 em = s_em_t[kk * (kTileX * kTY)];
                 // destinations of the voxel's z-run: two slots (a run of nsz subvoxels rarely meets a third voxel);
                 // B is the current one, A the one before; both are flushed at the end of the run, where every lane
                 // of the warp is there (the run length is CTA-uniform)
@@ -355,31 +355,32 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
 //     counters are derived from per-column counts, not per subvoxel.
 // Every destination is either proven equal to the contract's or computed by
 // it, so the result stays bit-identical to the oracle.
-template <int kNsz>
-__global__ void __launch_bounds__(kTileX * kTileY)
+// kNsz > 0: the z-run of a voxel is unrolled; kTY: rows of source columns per CTA (CTA = 32 x kTY columns)
+template <int kNsz, int kTY>
+__global__ void __launch_bounds__(kTileX * kTY)
 emtm_push_kernel(const __grid_constant__ PushParams P)
 {
     extern __shared__ AxisEntry s_map[];
     AxisEntry* sx = s_map;                               // [nsx][32]   (subvoxel-major: conflict-free 128-bit reads)
     AxisEntry* sy = sx + kTileX * P.nsx;                 // [4][nsy]
-    AxisEntry* sz = sy + kTileY * P.nsy;                 // [chunk_z * nsz]
+    AxisEntry* sz = sy + kTY * P.nsy;                 // [chunk_z * nsz]
     longlong2* s_em = reinterpret_cast<longlong2*>(sz + P.chunk_z * P.nsz);   // [chunk_z][128] (e_q, m_q) per voxel
-    float4* tile = reinterpret_cast<float4*>(s_em + P.chunk_z * kTileX * kTileY);   // [tile_cap] DVF nodes
+    float4* tile = reinterpret_cast<float4*>(s_em + P.chunk_z * kTileX * kTY);   // [tile_cap] DVF nodes
     __shared__ int s_okz;
     const int tid = threadIdx.y * kTileX + threadIdx.x;
     const int i = blockIdx.x * kTileX + threadIdx.x;
-    const int j = blockIdx.y * kTileY + threadIdx.y;
+    const int j = blockIdx.y * kTY + threadIdx.y;
     const int k0 = blockIdx.z * P.chunk_z;               // this CTA covers source voxels k0 .. k0 + kz_n - 1 along z
     const int kz_n = min(P.chunk_z, P.src.nz - k0);
-    const int n_x = kTileX * P.nsx, n_y = kTileY * P.nsy, n_z = kz_n * P.nsz;
+    const int n_x = kTileX * P.nsx, n_y = kTY * P.nsy, n_z = kz_n * P.nsz;
     if (tid == 0) s_okz = 0;
     __syncthreads();
-    for (int e = tid; e < n_x + n_y + n_z; e += kTileX * kTileY) {
+    for (int e = tid; e < n_x + n_y + n_z; e += kTileX * kTY) {
         if (e < n_x)
             s_map[e] = axis_map(P.src.ox, P.src.hx, blockIdx.x * kTileX + (e & (kTileX - 1)), e / kTileX, P.nsx,
                                 P.dvf.ox, P.dvf.hx, P.dvf.nx, P.ref.ox, P.ihdx);
         else if (e < n_x + n_y)
-            s_map[e] = axis_map(P.src.oy, P.src.hy, blockIdx.y * kTileY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
+            s_map[e] = axis_map(P.src.oy, P.src.hy, blockIdx.y * kTY + (e - n_x) / P.nsy, (e - n_x) % P.nsy, P.nsy,
                                 P.dvf.oy, P.dvf.hy, P.dvf.ny, P.ref.oy, P.ihdy);
         else {
             AxisEntry m = axis_map(P.src.oz, P.src.hz, k0 + (e - n_x - n_y) / P.nsz, (e - n_x - n_y) % P.nsz, P.nsz,
@@ -398,7 +399,7 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
     // memory when it fits: 16-byte asynchronous copies, in flight while the voxels' integer mass and energy are formed
     Tile T;
     {
-        const int nvx = min(kTileX, P.src.nx - blockIdx.x * kTileX), nvy = min(kTileY, P.src.ny - blockIdx.y * kTileY);
+        const int nvx = min(kTileX, P.src.nx - blockIdx.x * kTileX), nvy = min(kTY, P.src.ny - blockIdx.y * kTY);
         const int cx1 = sx[(P.nsx - 1) * kTileX + nvx - 1].cell, cy1 = sy[(nvy - 1) * P.nsy + P.nsy - 1].cell,
                   cz1 = sz[n_z - 1].cell;
         T.x0 = sx[0].cell & kCellNode; T.y0 = sy[0].cell & kCellNode; T.z0 = sz[0].cell & kCellNode;
@@ -409,7 +410,7 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
     const bool use_tile = P.dvf.nx > 1 && (long long)T.nx * T.ny * T.nz <= (long long)P.tile_cap;
     if (use_tile) {
         const int rows = T.ny * T.nz;
-        for (int r = tid >> 5; r < rows; r += (kTileX * kTileY) >> 5) {
+        for (int r = tid >> 5; r < rows; r += (kTileX * kTY) >> 5) {
             const int ty = r % T.ny, tz = r / T.ny;
             const float4* __restrict__ src = P.U + ((size_t)(T.z0 + tz) * P.dvf.ny + (T.y0 + ty)) * P.dvf.nx + T.x0;
             for (int x = tid & 31; x < T.nx; x += 32) {
@@ -430,7 +431,7 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
 #pragma unroll
         for (int kk = 0; kk < kChunkZMax; ++kk)
             if (kk < kz_n)
-                s_em[kk * (kTileX * kTileY) + tid] =
+                s_em[kk * (kTileX * kTY) + tid] =
                     make_longlong2(__double2ll_rn(__dmul_rn(__dmul_rn((double)rho[kk], (double)dose[kk]), 4294967296.0)),
                                    __double2ll_rn(__dmul_rn((double)rho[kk], 16777216.0)));
     }
@@ -454,8 +455,8 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
     {
         const float x0 = P.src.ox + (float)(blockIdx.x * kTileX) * P.src.hx;
         const float x1 = P.src.ox + (float)min(blockIdx.x * kTileX + kTileX, P.src.nx) * P.src.hx;
-        const float y0 = P.src.oy + (float)(blockIdx.y * kTileY) * P.src.hy;
-        const float y1 = P.src.oy + (float)min(blockIdx.y * kTileY + kTileY, P.src.ny) * P.src.hy;
+        const float y0 = P.src.oy + (float)(blockIdx.y * kTY) * P.src.hy;
+        const float y1 = P.src.oy + (float)min(blockIdx.y * kTY + kTY, P.src.ny) * P.src.hy;
         const float z0 = P.src.oz + (float)k0 * P.src.hz, z1 = P.src.oz + (float)(k0 + kz_n) * P.src.hz;
         interior = interior && (x0 - um.x >= P.ref.ox + 1.5f * P.ref.hx) &&
                    (x1 + um.x <= P.ref.ox + ((float)P.ref.nx - 1.5f) * P.ref.hx) &&
@@ -469,11 +470,11 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * P.nsy;
         if (use_tile) {
-            if (interior) push_columns<false, true, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, true, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
         } else {
-            if (interior) push_columns<false, false, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, false, kNsz>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            else          push_columns<true, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
         }
         n_dvf = (unsigned)(P.nsx * P.nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
         n_ref = eligible - landed;                            // mapped outside the reference grid (A4)
@@ -774,7 +775,7 @@ cudaError_t configure_accumulate(void)
     // the push kernel's axis maps + per-voxel (e_q, m_q) stage need up to 57 KB of dynamic shared memory at 64
     // subvoxels per axis.  A per-device attribute: pbs4d_create calls this for every context.
     cudaError_t e = cudaSuccess;
-    for (void (*k)(const PushParams) : { emtm_push_kernel<0>, emtm_push_kernel<2> })
+    for (void (*k)(const PushParams) : { emtm_push_kernel<0, 4>, emtm_push_kernel<0, 8>, emtm_push_kernel<2, 4> })
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     for (void (*k)(const PullParams) : { dim_pull_kernel<0, false>, dim_pull_kernel<0, true>, dim_pull_kernel<1, false>,
                                          dim_pull_kernel<1, true> })
@@ -818,20 +819,22 @@ void launch_emtm_push(const pbs4d_grid& src, const float* dose, const float* rho
     // With two z-subvoxels per voxel the CTA prologue weighs most: there the long column without the tile (the nodes
     // through L1) is best, 0.82 ms.
     P.chunk_z = nsz <= 2 ? kChunkZMax : 4;
-    dim3 b(kTileX, kTileY, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + kTileY - 1) / kTileY,
-                                 (src.nz + P.chunk_z - 1) / P.chunk_z);
+    // CTA shape: 32 x 8 columns from nsz = 3 on (the node box's halo and the CTA prologue are shared by twice the
+    // columns: config 4 n = 8 22.6 -> 21.1 ms, config 5 6.46 -> 6.25 ms), 32 x 4 below (n = 2: 0.735 against 0.749 ms)
+    const int ty = nsz >= 3 ? 8 : 4;
+    dim3 b(kTileX, ty, 1), g((src.nx + kTileX - 1) / kTileX, (src.ny + ty - 1) / ty, (src.nz + P.chunk_z - 1) / P.chunk_z);
     // shared memory: axis maps + (e_q, m_q) per voxel + the DVF tile.  The tile is sized for a field on the source
-    // grid's spacing ((32 + 2) x (4 + 2) x (chunk_z + 2) nodes) and shrunk so that the total stays under 60 KB.
-    const size_t fixed = (size_t)(kTileX * nsx + kTileY * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
-                         (size_t)P.chunk_z * kTileX * kTileY * sizeof(longlong2);
-    const size_t want = (size_t)(kTileX + 2) * (kTileY + 2) * (P.chunk_z + 2);
+    // grid's spacing ((32 + 2) x (ty + 2) x (chunk_z + 2) nodes) and shrunk so that the total stays under 60 KB.
+    const size_t fixed = (size_t)(kTileX * nsx + ty * nsy + P.chunk_z * nsz) * sizeof(AxisEntry) +
+                         (size_t)P.chunk_z * kTileX * ty * sizeof(longlong2);
+    const size_t want = (size_t)(kTileX + 2) * (ty + 2) * (P.chunk_z + 2);
     const size_t room = fixed < 60 * 1024 ? (60 * 1024 - fixed) / sizeof(float4) : 0;
     P.tile_cap = nsz <= 2 ? 0 : (int)std::min(want, room);
     const size_t smem = fixed + (size_t)P.tile_cap * sizeof(float4);
     // the two-subvoxel z-run of nsz = 2 is unrolled (config 4, 9 phases: 0.82 -> 0.73 ms); longer runs are not: the
     // unrolled body repeats the cell-change block and outgrows the instruction cache (nsz = 8: 22.5 -> 38 ms, nsz = 5:
     // 1.25 -> 1.63 ms).  (> 48 KB of shared memory possible: configure_accumulate() opted in)
-    void (*kernel)(const PushParams) = nsz == 2 ? emtm_push_kernel<2> : emtm_push_kernel<0>;
+    void (*kernel)(const PushParams) = nsz == 2 ? emtm_push_kernel<2, 4> : nsz >= 3 ? emtm_push_kernel<0, 8> : emtm_push_kernel<0, 4>;
     kernel<<<g, b, smem, st>>>(P);
 }
 

@@ -37,7 +37,7 @@ def test_no_unintended_packed_fma_in_the_contract_kernels():
     # the pull kernel: only the two fmas of the known-reciprocal division (x, y packed), in its two kFastDiv instantiations
     assert count("dim_pull_kernel", "FFMA2") == 4
     # push_columns<checked, tile> x 4: Axy, A12z per cell and the x/y and z estimates per subvoxel
-    assert count("emtm_push_kernel", "FFMA2") == 16 + 32       # runtime-nsz kernel + the nsz = 2 kernel (z-run unrolled twice)
+    assert count("emtm_push_kernel", "FFMA2") == 16 + 16 + 32  # runtime-nsz kernels (32 x 4 and 32 x 8 columns) + the nsz = 2 kernel (z-run unrolled twice)
     # the packed operations are really there (the kernels were built for sm_100a with f32x2)
     assert count("emtm_push_kernel", "FADD2") > 40 and count("dim_pull_kernel", "FADD2") > 4
     assert count("transport_kernel", "FFMA2") > 8
