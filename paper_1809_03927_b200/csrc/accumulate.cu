@@ -10,8 +10,12 @@
 // (PAPER.md:122-124).  Here the sums are int64 fixed point (order-independent, so the result is unique and
 // bit-reproducible), the subvoxel volume -- a common factor of Eq. 4 -- is dropped, and consecutive subvoxels of a
 // voxel that land in the same reference voxel are merged into one pair of red.global.add.u64.
-// Coordinate arithmetic is strict fp32: every operation is an explicit round-to-nearest intrinsic (never fused),
-// in the order fixed by DESIGN.md "Accumulation arithmetic"; this TU is also built with -fmad=false.
+// Coordinate arithmetic is strict fp32: every CONTRACT value is produced by explicit round-to-nearest operations
+// (scalar intrinsics or f32x2 pairs, never fused) in the order fixed by DESIGN.md "Accumulation arithmetic"; this TU is
+// also built with -fmad=false.  Two places use true fused operations by design, neither a contract value: the push's
+// folded index ESTIMATE (accepted only outside a derived tolerance of a voxel face, else the contract's chain decides)
+// and the pull's division by a known reciprocal (whose RESULT is the IEEE quotient).  tests/test_sass_contract.py pins
+// the FFMA2 count of the built kernels, because ptxas contracts packed mul + add on its own (see mad2_unfused).
 #include "internal.h"
 
 #include <cuda_runtime.h>
