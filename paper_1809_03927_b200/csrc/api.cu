@@ -53,6 +53,10 @@ struct PhaseLaunch {                     // per-phase segment table for the tran
 
 }  // namespace
 
+// layout of pbs4d_ctx::table: hu_pts | rho_pts (at most 64 floats each), then the 65536-double density LUT
+constexpr size_t kTableLutOffset = 2 * 64 * sizeof(float);
+constexpr size_t kTableBytes = kTableLutOffset + 65536 * sizeof(double);
+
 struct pbs4d_ctx {
     int device = 0;
     int sm_count = 148;
@@ -67,7 +71,7 @@ struct pbs4d_ctx {
     std::vector<bool> rho_valid;                         // [phase] density grid filled (run_plan_host fills active phases only)
     std::vector<cudaEvent_t> rho_ready;                  // [phase] density grid complete on the copy stream (run_plan_host)
     std::vector<bool> rho_pending;                       // [phase] the next transport launch must wait for rho_ready
-    DevBuf table;                                        // hu_pts | rho_pts
+    DevBuf table;                                        // hu_pts | rho_pts (<= 64 each) | 65536-entry density LUT
 
     // DVFs (a2)
     struct Dvf { bool set = false; int32_t ref = -1; pbs4d_grid grid{}; std::unique_ptr<DevBuf> disp; };
@@ -231,14 +235,15 @@ int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, 
     CU(cudaSetDevice(ctx->device));
     const pbs4d_grid& g = dose_grid ? *dose_grid : *ct;
     reset_phase_state(ctx, n_phases, g);
-    CU(ctx->table.ensure(2 * n_pts * sizeof(float)));
+    CU(ctx->table.ensure(kTableBytes));
     CU(cudaMemcpyAsync(ctx->table.p, hu_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->table.as<float>() + n_pts, rho_pts, n_pts * sizeof(float), cudaMemcpyHostToDevice,
                        ctx->stream));
     for (int p = 0; p < n_phases; ++p) {
         CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
-        launch_hu_to_density(*ct, hu_dev[p], dose_grid, n_pts, ctx->table.as<float>(),
-                             ctx->table.as<float>() + n_pts, ctx->rho[p]->as<float>(), ctx->stream);
+        launch_hu_to_density(*ct, hu_dev[p], dose_grid, n_pts, ctx->table.as<float>(), ctx->table.as<float>() + n_pts,
+                             rho_pts[0], reinterpret_cast<double*>(ctx->table.as<char>() + kTableLutOffset),
+                             ctx->rho[p]->as<float>(), ctx->stream);
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(ctx->stream));
@@ -874,7 +879,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
     const size_t ct_vox = (size_t)ct->nx * ct->ny * ct->nz;
     DevBuf& hu_dev = ctx->host_hu;
     CU(hu_dev.ensure(active.size() * ct_vox * sizeof(int16_t)));
-    CU(ctx->table.ensure(2 * n_pts * sizeof(float)));
+    CU(ctx->table.ensure(kTableBytes));
     // an early error return must not leave copies from the caller's host buffers in flight: armed before the first copy
     struct CopyGuard {
         cudaStream_t st[3] = { nullptr, nullptr, nullptr }; cudaEvent_t ev = nullptr; bool armed = false;
@@ -906,6 +911,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
         CU(ctx->rho[p]->ensure(ctx->nvox() * sizeof(float)));
         CU(cudaStreamWaitEvent(ctx->prep_stream, ctx->upload_done[2 * p], 0));
         launch_hu_to_density(*ct, dst, dose_grid, n_pts, ctx->table.as<float>(), ctx->table.as<float>() + n_pts,
+                             rho_pts[0], reinterpret_cast<double*>(ctx->table.as<char>() + kTableLutOffset),
                              ctx->rho[p]->as<float>(), ctx->prep_stream);
         CU(event_at(ctx->rho_ready, p));
         CU(cudaEventRecord(ctx->rho_ready[p], ctx->prep_stream));

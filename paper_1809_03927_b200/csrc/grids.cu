@@ -22,19 +22,48 @@ __device__ __forceinline__ double table_density(double hu, int n, const float* _
     return (double)rp[k] + f * ((double)rp[k + 1] - (double)rp[k]);
 }
 
-__global__ void hu_to_density_same_grid(long long nvox, const int16_t* __restrict__ hu, int n_pts,
-                                        const float* __restrict__ hp, const float* __restrict__ rp,
-                                        float* __restrict__ out)
+// HU is a 16-bit integer: the table function is evaluated once per possible value (65536 doubles, 512 KB, resident in
+// the L2) and the per-voxel kernels look it up -- the same double as evaluating it per voxel, without 42 million
+// double-precision divisions per phase of config 5.
+__global__ void density_lut_kernel(int n_pts, const float* __restrict__ hp, const float* __restrict__ rp,
+                                   double* __restrict__ lut)
+{
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;                     // 0 .. 65535  <->  HU -32768 .. 32767
+    if (v < 65536) lut[v] = table_density((double)(v - 32768), n_pts, hp, rp);
+}
+
+// HBM-bound: 2 B read + 4 B written per voxel; eight voxels per thread (one 128-bit load, two 128-bit stores)
+__global__ void __launch_bounds__(256)
+hu_to_density_same_grid(long long nvox, const int16_t* __restrict__ hu, const double* __restrict__ lut,
+                        float* __restrict__ out)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride)
-        out[i] = (float)table_density((double)hu[i], n_pts, hp, rp);
+    const long long n8 = nvox >> 3;
+    const bool aligned = ((reinterpret_cast<uintptr_t>(hu) | reinterpret_cast<uintptr_t>(out)) & 15) == 0;
+    long long done = 0;
+    if (aligned) {
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += stride) {
+            const int4 raw = __ldg(reinterpret_cast<const int4*>(hu) + i);
+            const int w[4] = { raw.x, raw.y, raw.z, raw.w };
+            float r[8];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                r[2 * k]     = (float)__ldg(lut + ((int)(short)(w[k] & 0xFFFF) + 32768));
+                r[2 * k + 1] = (float)__ldg(lut + ((w[k] >> 16) + 32768));
+            }
+            float4* o = reinterpret_cast<float4*>(out) + 2 * i;
+            o[0] = make_float4(r[0], r[1], r[2], r[3]);
+            o[1] = make_float4(r[4], r[5], r[6], r[7]);
+        }
+        done = n8 << 3;
+    }
+    for (long long i = done + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride)
+        out[i] = (float)__ldg(lut + ((int)hu[i] + 32768));
 }
 
 // dose-grid voxel = overlap-volume-weighted mean of the densities of the CT voxels it intersects
-__global__ void hu_to_density_resample(pbs4d_grid ct, pbs4d_grid dg, const int16_t* __restrict__ hu, int n_pts,
-                                       const float* __restrict__ hp, const float* __restrict__ rp,
-                                       float* __restrict__ out)
+__global__ void hu_to_density_resample(pbs4d_grid ct, pbs4d_grid dg, const int16_t* __restrict__ hu,
+                                       const double* __restrict__ lut, double rho_first, float* __restrict__ out)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -67,25 +96,50 @@ __global__ void hu_to_density_resample(pbs4d_grid ct, pbs4d_grid dg, const int16
                     wv *= ov > 0.0 ? ov : 0.0;
                 }
                 if (wv > 0.0) {
-                    acc  += wv * table_density((double)hu[((size_t)kz * cn[1] + ky) * cn[0] + kx], n_pts, hp, rp);
+                    acc  += wv * __ldg(lut + ((int)hu[((size_t)kz * cn[1] + ky) * cn[0] + kx] + 32768));
                     wsum += wv;
                 }
             }
-    out[((size_t)z * dg.ny + y) * dg.nx + x] = (float)(wsum > 0.0 ? acc / wsum : (double)rp[0]);
+    out[((size_t)z * dg.ny + y) * dg.nx + x] = (float)(wsum > 0.0 ? acc / wsum : rho_first);
 }
 
 // a7 / T12: D = Q 2^-k 1.602176634e-10 / (rho V_cm3)  [Gy]; optionally per proton.  A voxel without mass (never the
 // case for densities accepted by set_ct_phases / set_density_phases) gets dose 0 instead of 0/0.
-__global__ void finalize_dose_kernel(long long nvox, const float* __restrict__ rho, const long long* __restrict__ Q,
-                                     double inv_scale, double vol_cm3, double per_protons, float* __restrict__ dose)
+__device__ __forceinline__ float dose_of(long long q, float rho, double inv_scale, double vol_cm3, double per_protons)
+{
+    if (q == 0) return 0.0f;                 // 0 2^-k c / m = +0 for every finite m > 0 (and 0 for m <= 0): no arithmetic
+    const double mass = (double)rho * vol_cm3;
+    double D = (double)q * inv_scale * 1.602176634e-10 / mass;
+    if (per_protons > 0.0) D /= per_protons;
+    return mass > 0.0 ? (float)D : 0.0f;
+}
+
+// HBM-bound: 12 B read + 4 B written per voxel, two voxels per thread (128-bit load of the energies); a beam touches a
+// small part of the grid, so most voxels take the q == 0 exit and the double-precision divisions do not show
+__global__ void __launch_bounds__(256)
+finalize_dose_kernel(long long nvox, const float* __restrict__ rho, const long long* __restrict__ Q,
+                     double inv_scale, double vol_cm3, double per_protons, float* __restrict__ dose)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride) {
-        const double mass = (double)rho[i] * vol_cm3;
-        double D = (double)Q[i] * inv_scale * 1.602176634e-10 / mass;
-        if (per_protons > 0.0) D /= per_protons;
-        dose[i] = mass > 0.0 ? (float)D : 0.0f;
+    const long long n2 = nvox >> 1;
+    const bool aligned = ((reinterpret_cast<uintptr_t>(Q) & 15) | (reinterpret_cast<uintptr_t>(rho) & 7) |
+                          (reinterpret_cast<uintptr_t>(dose) & 7)) == 0;
+    long long done = 0;
+    if (aligned) {
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += stride) {
+            const longlong2 q = *(reinterpret_cast<const longlong2*>(Q) + i);
+            float2 d = make_float2(0.0f, 0.0f);
+            if (q.x | q.y) {
+                const float2 r = *(reinterpret_cast<const float2*>(rho) + i);
+                d.x = dose_of(q.x, r.x, inv_scale, vol_cm3, per_protons);
+                d.y = dose_of(q.y, r.y, inv_scale, vol_cm3, per_protons);
+            }
+            *(reinterpret_cast<float2*>(dose) + i) = d;
+        }
+        done = n2 << 1;
     }
+    for (long long i = done + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += stride)
+        dose[i] = dose_of(Q[i], rho[i], inv_scale, vol_cm3, per_protons);
 }
 
 // densities handed in directly (set_density_phases) must be finite and inside [kRhoMin, kRhoMax]: rho = 0 would give
@@ -183,15 +237,16 @@ int launch_validate_density(const float* rho, size_t n, int* flag_dev, cudaStrea
 }
 
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
-                          const float* hp, const float* rp, float* rho_out, cudaStream_t st)
+                          const float* hp, const float* rp, float rho_first, double* lut, float* rho_out, cudaStream_t st)
 {
+    density_lut_kernel<<<256, 256, 0, st>>>(n_pts, hp, rp, lut);             // 3 us; rebuilt per call: no state to keep
     if (!dose_grid) {
         const long long nvox = (long long)ct.nx * ct.ny * ct.nz;
-        const int blocks = (int)min((nvox + 255) / 256, (long long)sm_count_of_current_device() * 16);
-        hu_to_density_same_grid<<<blocks, 256, 0, st>>>(nvox, hu, n_pts, hp, rp, rho_out);
+        const int blocks = (int)min((nvox / 8 + 255) / 256 + 1, (long long)sm_count_of_current_device() * 16);
+        hu_to_density_same_grid<<<blocks, 256, 0, st>>>(nvox, hu, lut, rho_out);
     } else {
         dim3 b(32, 8, 1), g((dose_grid->nx + 31) / 32, (dose_grid->ny + 7) / 8, dose_grid->nz);
-        hu_to_density_resample<<<g, b, 0, st>>>(ct, *dose_grid, hu, n_pts, hp, rp, rho_out);
+        hu_to_density_resample<<<g, b, 0, st>>>(ct, *dose_grid, hu, lut, (double)rho_first, rho_out);
     }
 }
 

@@ -62,8 +62,11 @@ cudaError_t configure_accumulate(void);
 int launch_validate_density(const float* rho, size_t n, int* flag_dev, cudaStream_t st);
 #endif
 
+// lut: 65536 doubles of scratch owned by the caller (the table function per possible HU value; rebuilt by every call);
+// rho_first: rho_pts[0], the density of a dose voxel that overlaps no CT voxel
 void launch_hu_to_density(const pbs4d_grid& ct, const int16_t* hu, const pbs4d_grid* dose_grid, int32_t n_pts,
-                          const float* hu_pts_dev, const float* rho_pts_dev, float* rho_out, cudaStream_t st);
+                          const float* hu_pts_dev, const float* rho_pts_dev, float rho_first, double* lut,
+                          float* rho_out, cudaStream_t st);
 void launch_finalize_dose(const pbs4d_grid& g, const float* rho, const long long* Q, int32_t fixed_shift,
                           double per_protons, float* dose, cudaStream_t st);
 
