@@ -271,13 +271,13 @@ def run_pass(ctx, cfg, hu_dev, dvf_dev, rank, world, sum_grids=sum_energy_grids,
         extra = len(phases)                                                                        # second a7 launches
     ctx.set_shard(0, 1)
     n_src = int(ast["subvoxels"]) // (nvox * n_sub)                                               # phases pushed here
-    # kernels launched: HU->density per phase, DVF interleave per source phase, transport per phase with histories
+    # kernels launched: density table + HU->density per phase, DVF interleave per source phase, transport per phase with histories
     # here, dose finalize per phase run (twice when sharded), push per source phase pushed here, coverage flags +
     # accumulation finalize
     n_tr = sum(1 for st in sts if st["histories"] > 0)
     stats = dict(histories=n_hist, mc_steps=sum(st["steps"] for st in sts), reds=sum(st["scoring_atomics"] for st in sts),
                  transport_ms=t_ms, push_ms=ast["push_ms"], finalize_ms=ast["finalize_ms"], phases=len(phases),
-                 n_src=n_src, subvoxels=ast["subvoxels"], launches=P + n_dvf + n_tr + len(phases) + extra + n_src + 2,
+                 n_src=n_src, subvoxels=ast["subvoxels"], launches=2 * P + n_dvf + n_tr + len(phases) + extra + n_src + 2,
                  active=phases, src=src)
     return n_hist, out, stats
 
