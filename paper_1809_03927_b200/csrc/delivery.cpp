@@ -19,10 +19,29 @@ namespace {
 using u128 = unsigned __int128;
 constexpr int64_t kNsPerS = 1000000000;
 
+// quotient of two 128-bit values: the operands of this file nearly always fit in 64 bits (times in ns, distances in
+// um), where the hardware divide is several times faster than the 128-bit library routine; same result
+inline u128 div128(u128 a, u128 b)
+{
+    if (((a | b) >> 64) == 0) return (u128)((uint64_t)a / (uint64_t)b);
+    return a / b;
+}
+
 // floor(sqrt(v)) by Newton iteration on integers
 int64_t floor_sqrt(u128 v)
 {
     if (v == 0) return 0;
+    if ((v >> 62) == 0) {                              // the usual case, in 64-bit arithmetic (x + v / x < 2^63)
+        const uint64_t w = (uint64_t)v;
+        uint64_t x = (uint64_t)std::sqrt((double)w) + 2;
+        for (;;) {
+            const uint64_t y = (x + w / x) >> 1;
+            if (y >= x) break;
+            x = y;
+        }
+        while (x * x > w) --x;
+        return (int64_t)x;
+    }
     u128 x = (u128)std::sqrt((double)v) + 2;           // start at or above the root
     for (;;) {
         u128 y = (x + v / x) >> 1;
@@ -62,7 +81,7 @@ void allocate_histories(const std::vector<int64_t>& delivered, size_t nf, int32_
     u128 running = 0; int64_t edge_prev = 0;
     for (auto& sg : segments) {
         running += (u128)sg.protons;
-        const int64_t edge = total_histories ? (int64_t)(((u128)total_histories * running) / total) : 0;
+        const int64_t edge = total_histories ? (int64_t)div128((u128)total_histories * running, total) : 0;
         sg.first_history = edge_prev;
         sg.n_hist = edge - edge_prev;
         sg.weight = sg.n_hist > 0 ? (double)sg.protons / (double)sg.n_hist : 0.0;
@@ -122,11 +141,11 @@ int simulate_delivery_host(const std::vector<pbs4d_field>& fields, const std::ve
                         if (!clk.beam_allowed(t)) { t = clk.next_edge(t); continue; }      // gate closed: hold
                         const int64_t window = clk.next_edge(t) - t;                         // ns left in this phase
                         // protons leaving strictly before the edge: j * 1e9 / rate < window
-                        const u128 cap = ((u128)window * (u128)prm.protons_per_s + (kNsPerS - 1)) / kNsPerS;
+                        const u128 cap = div128((u128)window * (u128)prm.protons_per_s + (kNsPerS - 1), (u128)kNsPerS);
                         const int64_t n = cap < (u128)todo ? (int64_t)cap : todo;
                         delivered[(f * P + clk.phase(t)) * ns + s] += n;
                         todo -= n;
-                        t += (int64_t)(((u128)n * kNsPerS) / (u128)prm.protons_per_s);
+                        t += (int64_t)div128((u128)n * kNsPerS, (u128)prm.protons_per_s);
                     }
                 }
             }
