@@ -269,7 +269,12 @@ transport_kernel(const __grid_constant__ Params P)
 
     const unsigned lane = threadIdx.x & 31u;
     long long q_dep = 0;                                // rare tallies (incident, escaped, histories) go straight to
-    uint32_t n_steps = 0, n_red = 0;                    // shared memory; per-step ones stay in registers
+    uint32_t n_red = 0;                                 // shared memory; per-step ones stay in registers
+    // two per-thread values that are touched once per history live in shared memory, not in registers (the step loop sits
+    // at its register budget: one state register less was worth 1.4 %): the step count and the history's segment
+    __shared__ uint32_t s_nsteps[kThreads];
+    __shared__ int s_seg[kThreads];
+    s_nsteps[threadIdx.x] = 0u;
     const float hx = P.g.hx, hy = P.g.hy, hz = P.g.hz;
     const int   nx = P.g.nx, ny = P.g.ny, nz = P.g.nz;
 
@@ -325,7 +330,7 @@ transport_kernel(const __grid_constant__ Params P)
                         L.dx = S.dir[0] == 0.0f ? kTinyDir : S.dir[0];
                         L.dy = S.dir[1] == 0.0f ? kTinyDir : S.dir[1];
                         L.dz = S.dir[2] == 0.0f ? kTinyDir : S.dir[2];
-                        L.wq = S.weight_scaled; L.seg = tag;
+                        L.wq = S.weight_scaled; s_seg[threadIdx.x] = tag;
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.pend = 0;
                         L.rho = __ldg(P.rho + L.vox);
@@ -474,13 +479,13 @@ transport_kernel(const __grid_constant__ Params P)
 
             if (crossing || !alive) {
                 flush(P, L, q_dep, n_red);
-                if (!alive) n_steps += L.m;                                   // history absorbed: L.m = its step count
+                if (!alive) s_nsteps[threadIdx.x] += L.m;                     // history absorbed: L.m = its step count
                 if (alive) {
                     if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
                         atomicAdd((unsigned long long*)&s_tally[4],                            // left the grid
-                                  (unsigned long long)__double2ll_rn((double)L.E * P.segs[L.seg].weight_scaled_d));
+                                  (unsigned long long)__double2ll_rn((double)L.E * P.segs[s_seg[threadIdx.x]].weight_scaled_d));
                         alive = false;
-                        n_steps += L.m;
+                        s_nsteps[threadIdx.x] += L.m;
                     } else {
                         L.vox = (L.iz * ny + L.iy) * nx + L.ix;
                         L.rho = __ldg(P.rho + L.vox);
@@ -492,7 +497,7 @@ transport_kernel(const __grid_constant__ Params P)
     }
 
     // block-level tally reduction: warp shuffle, shared atomics, one global atomic per block and counter
-    long long v[6] = { 0, (long long)n_steps, 0, q_dep, 0, (long long)n_red };
+    long long v[6] = { 0, (long long)s_nsteps[threadIdx.x], 0, q_dep, 0, (long long)n_red };
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
         long long x = v[c];
