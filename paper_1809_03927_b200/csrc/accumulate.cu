@@ -234,8 +234,8 @@ template <bool kChecked, bool kTile, int kNsz, int kTY>
 __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntry* __restrict__ sxl,
                                              const AxisEntry* __restrict__ syl, const AxisEntry* __restrict__ sz,
                                              const longlong2* __restrict__ s_em_t, const float4* tile, const Tile T,
-                                             int kz_n, int okz, float htx, float hty, f32x2 tolz12, unsigned& eligible,
-                                             unsigned& landed)
+                                             int kz_n, float htx, float hty, f32x2 tolz12, unsigned& n_cols,
+                                             unsigned& dropped)
 {
     const int nsx = P.nsx, nsy = P.nsy, nsz = kNsz ? kNsz : P.nsz;      // kNsz > 0: the z-run is unrolled
     const int dnx = P.dvf.nx;
@@ -254,7 +254,7 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
         for (int a = 0; a < nsx; ++a) {
             const AxisEntry mx = sxl[a * kTileX];
             if (!(mx.cell & my.cell & kCellOk)) continue;                         // whole column outside the DVF extent
-            eligible += (unsigned)okz;
+            n_cols += 1u;
             // node (x0, y0) of z-node 0 of the field (global) or of the tile
             const int col_t = ((my.cell & kCellNode) - T.y0) * row + ((mx.cell & kCellNode) - T.x0) - T.z0 * sz_stride;
             const float4* __restrict__ col = P.U + ((size_t)(my.cell & kCellNode) * dnx + (mx.cell & kCellNode));
@@ -274,7 +274,8 @@ __device__ __forceinline__ void push_columns(const PushParams& P, const AxisEntr
                     if (dst >= 0) {
                         atomicAdd(P.E + dst, (unsigned long long)em.x * cnt);
                         atomicAdd(P.M + dst, (unsigned long long)em.y * cnt);
-                        landed += cnt;
+                    } else {
+                        dropped += cnt;                  // mapped outside the reference grid (A4): the rare side counts
                     }
                 };
 #pragma unroll
@@ -470,18 +471,20 @@ emtm_push_kernel(const __grid_constant__ PushParams P)
                    (z1 + um.z <= P.ref.oz + ((float)P.ref.nz - 1.5f) * P.ref.hz);
     }
     if (mine) {
-        unsigned landed = 0, eligible = 0;
+        unsigned dropped = 0, n_cols = 0;                    // subvoxels the flushes dropped; columns inside the DVF's x/y extent
         const AxisEntry* sxl = sx + threadIdx.x;
         const AxisEntry* syl = sy + threadIdx.y * P.nsy;
         if (use_tile) {
-            if (interior) push_columns<false, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, htx, hty, tolz12, n_cols, dropped);
+            else          push_columns<true, true, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, htx, hty, tolz12, n_cols, dropped);
         } else {
-            if (interior) push_columns<false, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
-            else          push_columns<true, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, okz, htx, hty, tolz12, eligible, landed);
+            if (interior) push_columns<false, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, htx, hty, tolz12, n_cols, dropped);
+            else          push_columns<true, false, kNsz, kTY>(P, sxl, syl, sz, s_em + tid, tile, T, kz_n, htx, hty, tolz12, n_cols, dropped);
         }
-        n_dvf = (unsigned)(P.nsx * P.nsy * n_z) - eligible;   // subvoxel centres outside the DVF grid's extent (A3)
-        n_ref = eligible - landed;                            // mapped outside the reference grid (A4)
+        // subvoxel centres outside the DVF grid's extent (A3): whole columns (x or y outside) and, in the walked columns, the
+        // NaN-coded z-subvoxels; mapped outside the reference grid (A4): what the flushes dropped, minus those z-subvoxels
+        n_dvf = (unsigned)(P.nsx * P.nsy * n_z) - n_cols * (unsigned)okz;
+        n_ref = dropped - n_cols * (unsigned)(n_z - okz);
     }
     // drop counters: warp-reduce, one atomic per warp
 #pragma unroll
