@@ -169,6 +169,31 @@ def test_density_kernels_bit_exact(ctx):
             assert (rho.cpu().numpy() == want).all()
 
 
+def test_density_and_dose_kernels_on_odd_sizes_and_the_whole_hu_range(ctx):
+    # a grid whose voxel count is odd (the vectorised kernels' scalar tails), HU values over the whole int16 range
+    # (the 65536-entry table; values beyond the table ends are clamped, A4) and a phase pointer that is not 16-byte aligned
+    rng = np.random.default_rng(31)
+    cfg = synth.config2(n_hist=10)
+    g = synth.make_grid((5, 7, 13), (2.0, 2.0, 2.0))
+    hu = rng.integers(-32768, 32768, (5 * 7 * 13 + 3,), dtype=np.int64).astype(np.int16)
+    hu[:8] = (-32768, 32767, -1000, -1001, 0, 1000, 1001, -999)
+    hu_dev = torch.from_numpy(hu).cuda()
+    for off in (0, 3):                                                    # off = 3: a 6-byte offset into the buffer
+        phase = hu_dev[off:off + 5 * 7 * 13].view(5, 7, 13)
+        ctx.set_ct_phases(g, [phase], None)
+        fields = synth.make_field((0, 0, 1), (1, 0, 0), (0, 1, 0), (13.0, 7.0, 0.0))
+        spots = cfg["spots"][:1].copy(); spots["x_mm"] = 0.0; spots["y_mm"] = 0.0
+        ctx.set_plan_spots(fields, spots)
+        ctx.simulate_delivery(cfg["deliv"], 2000)
+        dose, rho, stats = ctx.mc_dose_phase(0, 7, want_dose=True, want_rho=True)
+        want = orc.hu_to_density(g, hu[off:off + 5 * 7 * 13].reshape(5, 7, 13), None)
+        assert (rho.cpu().numpy() == want).all()
+        # the dose of a voxel without energy is +0, and the grid holds exactly as many non-zero doses as non-zero energies
+        Q = ctx.get_phase_energy(0).cpu().numpy()
+        d = dose.cpu().numpy()
+        assert ((d != 0) == (Q != 0)).all() and (Q != 0).any() and (Q == 0).any()
+
+
 def test_call_order_and_argument_errors(ctx):
     c = synth.config4(n=16, n_phases=2)
     fresh = binding.Context(0)
