@@ -327,6 +327,38 @@ typedef struct {
 int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, const float* delta_dev, float* rf_dev, float* disp_dev,
                     pbs4d_grid* grid_out);
 
+/* ---- a1 without any allocation ("converting Hounsfield Units to material density") ----
+ * For callers that cannot call cudaMalloc: a process whose own memory pool already owns almost all of the GPU (a
+ * planning server's caching allocator, PyTorch) has nothing left for an allocation made by a library, and a loop with a
+ * latency budget cannot take the driver locks of cudaMalloc or the device-wide wait of cudaFree.  This call needs no
+ * context (pbs4d_create allocates) and makes no cudaMalloc, cudaFree or other allocating call, on any invocation.
+ *
+ *   rho_dev[i] = (float) table(hu_dev[i]),  i < n_voxels;  table = the piecewise-linear function through
+ *   (hu_pts[k], rho_pts[k]), clamped at its ends, evaluated in double -- bit for bit what pbs4d_set_ct_phases computes
+ *   when dose_grid == NULL (no resampling here).
+ *
+ * hu_dev (int16, n_voxels), rho_dev (fp32, n_voxels): DEVICE pointers on the calling thread's CURRENT device, caller's
+ * buffers, any alignment (16-byte aligned pointers take the vector path).  hu_pts, rho_pts: HOST, n_pts entries, HU
+ * strictly ascending, densities > 0; read before the call returns.  cuda_stream: cudaStream_t or NULL.
+ * Limits: 2 <= n_pts <= PBS4D_NOALLOC_MAX_TABLE_PTS, 0 <= n_voxels <= PBS4D_NOALLOC_MAX_VOXELS; anything beyond is
+ * refused with PBS4D_ERR_ARG before any work is queued (nothing can grow).
+ * Scratch: PBS4D_NOALLOC_SCRATCH_BYTES (512 KiB: the table function at each of the 65536 int16 values) in a static
+ * device array inside the library; every GPU that loads the library holds it until the process exits.  All calls on a
+ * device share it.  Each call rewrites the whole array before reading it, so nothing is carried from call to call and
+ * calls queued on ONE stream may follow each other freely; calls that can overlap on the GPU (different streams without
+ * an event between them, or several host threads on one device) race on it and give undefined densities.
+ * The first call on each device also looks up the scratch's device address (cudaGetSymbolAddress, which loads the
+ * module): make that first call before starting any stream capture on that device, e.g. once at start-up with
+ * n_voxels = 0.
+ * Unlike the context calls this one only ENQUEUES (two kernels on cuda_stream) and returns: the caller synchronises.
+ * Errors: the return code, and a message in err[err_cap] (caller's buffer, optional; always terminated, "" on
+ * success).  PBS4D_ERR_CUDA without a device -- there is no CPU fallback. */
+#define PBS4D_NOALLOC_MAX_TABLE_PTS   64
+#define PBS4D_NOALLOC_MAX_VOXELS      2000000000LL
+#define PBS4D_NOALLOC_SCRATCH_BYTES   524288
+int pbs4d_hu_to_density_noalloc(const int16_t* hu_dev, int64_t n_voxels, int32_t n_pts, const float* hu_pts,
+                                const float* rho_pts, float* rho_dev, void* cuda_stream, char* err, int32_t err_cap);
+
 /* In-run roofline probes (BASELINE.json north_star: throughput is reported "as achieved fraction of the FP32-issue,
  * L2-atomic and HBM roofline measured by in-run microbenchmarks").  Each probe launches a small kernel of its own on
  * the context's stream, times it with CUDA events (best of 3-5 after a warm-up) and writes one number to *value:

@@ -35,7 +35,8 @@ EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_ph
            "pbs4d_set_dvf_pull", "pbs4d_accumulate_dim", "pbs4d_simulate_delivery_ext", "pbs4d_simulate_delivery_ext_host",
            "pbs4d_build_dvf", "pbs4d_shard_window", "pbs4d_set_shard", "pbs4d_phase_energy_ptr",
            "pbs4d_finalize_phase_dose", "pbs4d_accumulate_push", "pbs4d_accumulator_ptrs", "pbs4d_accumulate_finalize",
-           "pbs4d_sample_delivery_trial", "pbs4d_simulate_delivery_trial", "pbs4d_run_trials"]
+           "pbs4d_sample_delivery_trial", "pbs4d_simulate_delivery_trial", "pbs4d_run_trials",
+           "pbs4d_hu_to_density_noalloc"]
 
 
 class PhaseLists(C.Structure):
@@ -135,6 +136,40 @@ def shard_window(n_hist, rank, world):
     if rc != 0:
         raise RuntimeError(f"pbs4d_shard_window: error {rc}")
     return int(b.value), int(c.value)
+
+
+NOALLOC_MAX_TABLE_PTS, NOALLOC_MAX_VOXELS, NOALLOC_SCRATCH_BYTES = 64, 2_000_000_000, 524288
+
+
+def hu_to_density_noalloc(hu, out, hu_pts=(-1000.0, 0.0, 1000.0), rho_pts=(0.001, 1.0, 1.6), stream=None):
+    """pbs4d_hu_to_density_noalloc: HU -> density for callers that must not allocate device memory (a process whose
+    memory pool owns the GPU, a latency-bound loop); no context, no cudaMalloc / cudaFree inside.  `hu` (int16) and `out`
+    (float32, same element count) are the caller's contiguous CUDA tensors on the current device; the call only
+    enqueues on `stream` (default: torch's current stream) -- synchronise before reading `out`.  The 512 KiB scratch
+    is a static device array shared by all calls on a device: calls on one stream may follow each other, calls that
+    overlap on the GPU race.  The first call on a device also does the one-time set-up (make it before any stream
+    capture).  Without tensors (`hu`, `out` = None) the call runs with n_voxels = 0: argument checks and set-up only.
+    Raises RuntimeError with the library's message on failure (too many table points, too many voxels, ...)."""
+    import torch
+    if hu is None:
+        n, hu_ptr, out_ptr = 0, None, None
+    else:
+        if hu.dtype != torch.int16 or out.dtype != torch.float32 or not hu.is_cuda or not out.is_cuda or \
+                not hu.is_contiguous() or not out.is_contiguous() or hu.numel() != out.numel():
+            raise ValueError("hu_to_density_noalloc: hu int16 / out float32 contiguous CUDA tensors of one size")
+        n, hu_ptr, out_ptr = hu.numel(), C.c_void_p(hu.data_ptr()), C.c_void_p(out.data_ptr())
+    hp = np.ascontiguousarray(hu_pts, np.float32)
+    rp = np.ascontiguousarray(rho_pts, np.float32)
+    if hp.ndim != 1 or hp.shape != rp.shape:
+        raise ValueError("hu_to_density_noalloc: hu_pts and rho_pts must be 1-D and of one length")
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    err = C.create_string_buffer(256)
+    rc = load().pbs4d_hu_to_density_noalloc(hu_ptr, C.c_int64(n), C.c_int32(len(hp)), _np(hp), _np(rp), out_ptr,
+                                            C.c_void_p(stream), err, C.c_int32(len(err)))
+    if rc != 0:
+        raise RuntimeError(f"pbs4d error {rc}: {err.value.decode()}")
+    return out
 
 
 class _DevView:

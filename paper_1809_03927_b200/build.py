@@ -1,6 +1,6 @@
 """Build libpbs4d.so (the C-ABI library of include/pbs4d.h) in-tree with nvcc for sm_100a.
 
-transport.cu is built with the default FMA contraction; grids.cu and accumulate.cu with -fmad=false (their
+transport.cu is built with the default FMA contraction; grids.cu, noalloc.cu and accumulate.cu with -fmad=false (their
 arithmetic must round operation by operation -- DESIGN.md "Accumulation arithmetic").
 """
 import os
@@ -14,6 +14,7 @@ LIB = os.path.join(HERE, "libpbs4d.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
 UNITS = [("api.cu", []), ("transport.cu", []), ("grids.cu", ["-fmad=false"]), ("accumulate.cu", ["-fmad=false"]), ("roofline.cu", []),
+         ("noalloc.cu", ["-fmad=false"]),
          ("delivery.cpp", []), ("tables.cpp", []), ("trials.cpp", [])]
 
 
