@@ -31,7 +31,8 @@ extern "C" {
 
 typedef struct pbs4d_ctx pbs4d_ctx;      /* opaque; owns all internal host/device memory */
 
-/* at most 4e6 voxels per axis and 2e9 in total */
+/* at most 4 000 000 x 262 140 x 65 535 voxels (x, y, z: kernel launch geometry) and fewer than 2e9 in total;
+ * anything else is refused with PBS4D_ERR_ARG by the call that receives the grid */
 typedef struct { int32_t nx, ny, nz; float hx, hy, hz, ox, oy, oz; } pbs4d_grid;
 
 /* A treatment field: parallel beam along dir; (eu, ev) span the beam's-eye-view plane through ref.
@@ -190,7 +191,10 @@ int pbs4d_sample_delivery_trial(const pbs4d_trial_spec* spec, int32_t trial, int
                                 int32_t* start_phase, int64_t* cycle_period_ns, int64_t* layer_switch_ns,
                                 pbs4d_delivery_params* prm_out, pbs4d_delivery_ext* ext_out);
 
-/* a3 for one trial: sample it, start every field in its sampled phase and run the extended delivery simulation. */
+/* a3 for one trial: sample it, start every field in its sampled phase and run the extended delivery simulation (always
+ * the extended one: with ext == NULL the central values are the base model's, which the extended simulator reproduces).
+ * The plan kept by the context is not changed: the planned starting phases are back when the call returns, also after
+ * an error; only the segment lists in the context are the trial's. */
 int pbs4d_simulate_delivery_trial(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, int32_t trial,
                                   const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
                                   uint64_t total_histories, pbs4d_phase_lists* out, int64_t* n_fills);
@@ -255,7 +259,9 @@ int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, in
 int pbs4d_shard_window(int64_t n_hist, int32_t rank, int32_t world, int64_t* begin, int64_t* count);
 
 /* Subsequent mc_dose_phase(s) transport only this rank's slice of every phase (default rank 0 of 1 = everything).
- * Stats then count the slice; doses kept by the context are partial until the grids have been summed. */
+ * Stats then count the slice; doses kept by the context are partial until the grids have been summed.  The setting
+ * stays until changed; pbs4d_run_plan_host and pbs4d_run_trials, which contain no exchange step, return
+ * PBS4D_ERR_ORDER while world > 1. */
 int pbs4d_set_shard(pbs4d_ctx* ctx, int32_t rank, int32_t world);
 
 /* Device pointer to the context's own int64 energy grid [z][y][x] of `phase` (valid until the next set_ct_phases /

@@ -144,12 +144,24 @@ int on_exception(pbs4d_ctx* c) noexcept
 
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
 
-bool grid_ok(const pbs4d_grid* g)
+// nullptr for a usable grid, else what is wrong with it.  The per-axis limits are those of the launch geometry: the
+// accumulation kernels put ceil(ny / 4) CTAs on grid.y and ceil(nz / 4) on grid.z, the resampling density kernel nz on
+// grid.z (each at most 65535), and rows (ny * nz) go on grid.x, which the total bounds.
+const char* grid_defect(const pbs4d_grid* g)
 {
-    return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->hx > 0.0f && g->hy > 0.0f && g->hz > 0.0f &&
-           std::isfinite(g->ox) && std::isfinite(g->oy) && std::isfinite(g->oz) &&
-           g->nx <= 4000000 && g->ny <= 4000000 && g->nz <= 4000000 && (double)g->nx * g->ny * g->nz < 2.0e9;
+    if (!g) return "null grid";
+    if (!(g->nx > 0 && g->ny > 0 && g->nz > 0)) return "grid needs at least one voxel per axis";
+    if (!(g->hx > 0.0f && g->hy > 0.0f && g->hz > 0.0f) || !std::isfinite(g->hx) || !std::isfinite(g->hy) ||
+        !std::isfinite(g->hz))
+        return "grid spacings must be positive and finite";
+    if (!std::isfinite(g->ox) || !std::isfinite(g->oy) || !std::isfinite(g->oz)) return "grid origin must be finite";
+    if (g->nx > 4000000 || g->ny > 262140 || g->nz > 65535)
+        return "grid too long: at most 4000000 x 262140 x 65535 voxels (x, y, z)";
+    if (!((double)g->nx * g->ny * g->nz < 2.0e9)) return "grid too large: fewer than 2e9 voxels in total";
+    return nullptr;
 }
+
+bool grid_ok(const pbs4d_grid* g) { return grid_defect(g) == nullptr; }
 
 void reset_phase_state(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid& g)
 {
@@ -224,8 +236,9 @@ int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, 
                         const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
-    if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_dev || (dose_grid && !grid_ok(dose_grid)) ||
-        n_pts < 2 || n_pts > 64 || !hu_pts || !rho_pts)
+    if (const char* why = grid_defect(ct)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_ct_phases: ct: ") + why);
+    if (dose_grid) if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_ct_phases: dose_grid: ") + why);
+    if (n_phases < 1 || n_phases > 32 || !hu_dev || n_pts < 2 || n_pts > 64 || !hu_pts || !rho_pts)
         return fail(ctx, PBS4D_ERR_ARG, "set_ct_phases: bad argument");
     for (int i = 0; i < n_pts; ++i) {
         if (!(rho_pts[i] > 0.0f) || (i && !(hu_pts[i] > hu_pts[i - 1])))
@@ -257,7 +270,8 @@ int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid*
                              const float* const* rho_dev) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
-    if (n_phases < 1 || n_phases > 32 || !grid_ok(dose_grid) || !rho_dev)
+    if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_density_phases: ") + why);
+    if (n_phases < 1 || n_phases > 32 || !rho_dev)
         return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: bad argument");
     for (int p = 0; p < n_phases; ++p) if (!rho_dev[p]) return fail(ctx, PBS4D_ERR_ARG, "set_density_phases: null phase");
     CU(cudaSetDevice(ctx->device));
@@ -288,8 +302,9 @@ static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const c
     if (!ctx) return PBS4D_ERR_ARG;
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, std::string(who) + ": call set_ct_phases/set_density_phases first");
     if (src_phase < 0 || src_phase >= ctx->n_phases || ref_phase < 0 || ref_phase >= ctx->n_phases ||
-        src_phase == ref_phase || !grid_ok(dvf_grid) || !disp_dev)
+        src_phase == ref_phase || !disp_dev)
         return fail(ctx, PBS4D_ERR_ARG, std::string(who) + ": bad argument");
+    if (const char* why = grid_defect(dvf_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string(who) + ": dvf_grid: " + why);
     CU(cudaSetDevice(ctx->device));
     auto& d = table[src_phase];
     if (!d.disp) d.disp.reset(new DevBuf);
@@ -785,6 +800,13 @@ extern "C" int pbs4d_simulate_delivery_trial(pbs4d_ctx* ctx, const pbs4d_trial_s
     pbs4d_delivery_params p{}; pbs4d_delivery_ext x{};
     const int rc = sample_trial_host(*spec, trial, nf, *prm, central, start.data(), cycles.data(), resets.data(), p, x);
     if (rc != PBS4D_OK) return fail(ctx, rc, "simulate_delivery_trial: bad trial specification");
+    // the sampled starting phases are this trial's, not the plan's: the planned ones come back when the call ends,
+    // whether or not the simulation succeeds (the segment lists it leaves in the context are the trial's)
+    struct RestoreStartPhases {
+        std::vector<pbs4d_field>& fields; std::vector<int32_t> planned;
+        explicit RestoreStartPhases(std::vector<pbs4d_field>& f) : fields(f) { for (const auto& e : f) planned.push_back(e.start_phase); }
+        ~RestoreStartPhases() { for (size_t f = 0; f < planned.size() && f < fields.size(); ++f) fields[f].start_phase = planned[f]; }
+    } restore(ctx->fields);
     for (int32_t f = 0; f < nf; ++f) ctx->fields[f].start_phase = start[f];
     return pbs4d_simulate_delivery_ext(ctx, &p, &x, total_histories, out, n_fills);
 }
@@ -799,6 +821,9 @@ extern "C" int pbs4d_run_trials(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, in
     if (!spec || !prm || !dose4d_dev || first < 0 || count < 1 || first + count > spec->n_trials)
         return fail(ctx, PBS4D_ERR_ARG, "run_trials: bad argument");
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "run_trials: no densities (set_ct_phases)");
+    if (ctx->shard_world != 1)                              // no exchange happens in here: the doses would be partial
+        return fail(ctx, PBS4D_ERR_ORDER, "run_trials: history sharding is on (set_shard(0, 1) first); a sharded run "
+                                          "needs the caller's sum over ranks between transport and accumulation");
     if (ref_phase < 0 || ref_phase >= ctx->n_phases) return fail(ctx, PBS4D_ERR_ARG, "run_trials: bad reference phase");
     for (int32_t t = 0; t < count; ++t) {
         if (!dose4d_dev[t]) return fail(ctx, PBS4D_ERR_ARG, "run_trials: null output buffer");
@@ -842,6 +867,9 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
                                    uint64_t* h2d_bytes, double* seconds) try
 {
     if (!ctx) return PBS4D_ERR_ARG;
+    if (const char* why = grid_defect(ct)) return fail(ctx, PBS4D_ERR_ARG, std::string("run_plan_host: ct: ") + why);
+    if (dose_grid) if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("run_plan_host: dose_grid: ") + why);
+    if (disp_host) if (const char* why = grid_defect(dvf_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("run_plan_host: dvf_grid: ") + why);
     if (n_phases < 1 || n_phases > 32 || !grid_ok(ct) || !hu_host || !prm || !dose4d_host || ref_phase < 0 ||
         ref_phase >= n_phases || prm->n_phases != n_phases || (disp_host && !grid_ok(dvf_grid)) ||
         (dose_grid && !grid_ok(dose_grid)) || n_pts < 2 || n_pts > 64 || !hu_pts || !rho_pts)
@@ -851,6 +879,9 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
             return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: table must ascend in HU with positive densities");
     for (int p = 0; p < n_phases; ++p)
         if (!hu_host[p]) return fail(ctx, PBS4D_ERR_ARG, "run_plan_host: null CT phase");
+    if (ctx->shard_world != 1)                              // no exchange happens in here: the dose would be partial
+        return fail(ctx, PBS4D_ERR_ORDER, "run_plan_host: history sharding is on (set_shard(0, 1) first); a sharded run "
+                                          "needs the caller's sum over ranks between transport and accumulation");
     using clk = std::chrono::steady_clock;
     auto sec = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
     CU(cudaSetDevice(ctx->device));

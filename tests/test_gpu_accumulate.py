@@ -207,6 +207,16 @@ def test_call_order_and_argument_errors(ctx):
         fresh.accumulate_subvoxel(0, (2, 2, 2))                      # no doses yet
     with pytest.raises(RuntimeError, match="-2"):
         fresh.mc_dose_phase(0, 1)                                    # no delivery yet
+    # grids longer than the kernels' launch geometry allows are refused by the call that receives them, with a message
+    # that says so (not by a failed launch later); the buffers are never touched
+    tiny = torch.ones(8, dtype=torch.float32, device="cuda")
+    for shape in ((1, 262141, 1), (65536, 1, 1)):
+        with pytest.raises(RuntimeError, match="-1.*grid too long"):
+            fresh.set_density_phases(synth.make_grid(shape, (2.0, 2.0, 2.0)), [tiny])
+        with pytest.raises(RuntimeError, match="-1.*dvf_grid: grid too long"):
+            fresh.set_dvf(1, 0, synth.make_grid(shape, (2.0, 2.0, 2.0)), tiny)
+    with pytest.raises(RuntimeError, match="-1.*2e9"):
+        fresh.set_density_phases(synth.make_grid((2000, 2000, 2000), (2.0, 2.0, 2.0)), [tiny])
     fresh.close()
 
 

@@ -110,7 +110,19 @@ def test_more_ranks_than_histories_and_bad_arguments(ctx):
         ctx.set_shard(3, 3)
     with pytest.raises(RuntimeError):
         ctx.set_shard(-1, 2)
+    # the whole-path entry points contain no exchange step: with sharding on they would hand back a dose built from a
+    # slice of the histories, so they refuse (PBS4D_ERR_ORDER) until the shard is reset
+    ctx.set_shard(1, 2)
+    out = np.zeros(synth.grid_shape(cfg["ct_grid"]), np.float32)
+    with pytest.raises(RuntimeError, match="-2.*sharding"):
+        ctx.run_plan_host(cfg["ct_grid"], [cfg["hu"][0]], None, None, None, 0, cfg["fields"], cfg["spots"], cfg["deliv"],
+                          cfg["histories"], 7, (1, 1, 1), out)
+    spec = dict(seed=1, n_trials=2, n_cycles=0)
+    with pytest.raises(RuntimeError, match="-2.*sharding"):
+        ctx.run_trials(spec, 0, 1, cfg["deliv"], cfg["histories"], 7, 0, (1, 1, 1))
     ctx.set_shard(0, 1)
+    _, _, s = ctx.mc_dose_phase(0, 7, want_dose=False)         # the refused calls left the context as it was
+    assert s["histories"] == 5 and torch.equal(ctx.get_phase_energy(0), Q0)
 
 
 def test_density_validation_rejects_zero_and_nonfinite(ctx):

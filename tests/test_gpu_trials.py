@@ -28,16 +28,25 @@ def test_run_trials_equals_stepwise_and_oracle_delivery():
         if cfg["dvf"][p] is not None:
             ctx.set_dvf(p, cfg["ref_phase"], cfg["dvf_grid"], torch.from_numpy(cfg["dvf"][p]).cuda())
     ctx.set_plan_spots(cfg["fields"], cfg["spots"])
+    planned = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
     outs, res = ctx.run_trials(SPEC, 0, 25, cfg["deliv"], cfg["histories"], 1000, cfg["ref_phase"], cfg["subvox"], **EXT)
     assert len(outs) == 25 and all(r["histories"] == cfg["histories"] for r in res)
     assert all(1 <= r["phases_run"] <= 5 and r["fills"] >= 75 and r["delivery_ns"] > 0 for r in res)
     sums = [float(o.double().sum()) for o in outs]
     assert len(set(sums)) == 25 and min(sums) > 0                       # 25 different 4D doses
     assert len(set(r["delivery_ns"] for r in res)) == 25
+    # the trials start the fields in sampled phases; the plan itself must come out of the loop untouched
+    again = ctx.simulate_delivery(cfg["deliv"], cfg["histories"])
+    assert again["segments"].tobytes() == planned["segments"].tobytes()
+    assert (again["field_time_ns"] == planned["field_time_ns"]).all()
     for trial in (0, 7, 24):
         d = ctx.simulate_delivery_trial(SPEC, trial, cfg["deliv"], cfg["histories"], **EXT)
         o = orc.sample_trial(SPEC, trial, 3, cfg["deliv"], **EXT)
         f = cfg["fields"].copy(); f["start_phase"] = o["start_phase"]
+        if trial == 7:
+            assert (o["start_phase"] != cfg["fields"]["start_phase"]).any()   # a trial that does move the start
+            assert ctx.simulate_delivery(cfg["deliv"], cfg["histories"])["segments"].tobytes() == planned["segments"].tobytes()
+            d = ctx.simulate_delivery_trial(SPEC, trial, cfg["deliv"], cfg["histories"], **EXT)
         segs, tt, _, fills = orc.simulate_delivery_ext(f, cfg["spots"], o["prm"], cfg["histories"], **o["ext"])
         assert d["segments"].tobytes() == np.ascontiguousarray(segs).tobytes() and d["fills"] == fills
         assert res[trial]["delivery_ns"] == int(tt.max())
