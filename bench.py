@@ -133,7 +133,7 @@ def oracle_sample(cfg, budget_hist):
         t_tr += time.time() - t1
         n += int(st["histories"])
     wall = time.time() - t0
-    cores = len(os.sched_getaffinity(0))
+    cores = orc.threads()                                       # the threads the oracle's history loop ran on
     return n / wall, cores, (f"{n} histories of the {cfg['name']} plan over its delivered phases "
                              f"(delivery + HU->density + transport; {wall:.1f} s wall, transport {t_tr:.1f} s)")
 

@@ -120,6 +120,11 @@ def fixed_shift(segs, spots):
     return int(lib().orc_fixed_shift(C.c_int64(len(segs)), _p(segs), _p(spots)))
 
 
+def threads():
+    """threads the oracle's history loop runs on (OpenMP)"""
+    return int(lib().orc_threads())
+
+
 def transport(grid, rho, fields, spots, segs, seed, shift, flags=0, probe_faces=None, trace=None):
     """T1-T12 over the given segments.  Returns (Q int64 [z,y,x], stats record, probe_xy or None, stop_xyz or None).
     trace = (hist_base, hist_count) enables stop_xyz (and probe_xy when probe_faces is given)."""

@@ -110,6 +110,9 @@ int32_t orc_fixed_shift(int64_t n_segs, const orc_segment* segs, const orc_spot*
  * voxel k-1 and k); probe_xy[(p*H + g_local)*2 + {0,1}] receives x,y of history g_local = g - hist_base at its first +z crossing
  * of that face (NaN if never).  stop_xyz[g_local*3..] (optional) receives the position where the history ended
  * (absorbed) or NaN if it escaped. */
+/* number of threads orc_transport's history loop runs on (OpenMP; OMP_NUM_THREADS) */
+int orc_threads(void);
+
 int orc_transport(const orc_grid* grid, const float* rho,
                   int32_t n_fields, const orc_field* fields, const orc_spot* spots,
                   int64_t n_segs, const orc_segment* segs,

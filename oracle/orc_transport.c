@@ -9,6 +9,9 @@
 #include <math.h>
 #include <string.h>
 #include <stdlib.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 static const double E_CUT_ = 0.5;
 static const double S_MAX_ = 1.0;          /* mm */
@@ -184,6 +187,16 @@ static void one_history(const orc_grid* G, const float* rho, const orc_field* F,
     if (stop_xyz) { stop_xyz[gl*3] = r[0]; stop_xyz[gl*3+1] = r[1]; stop_xyz[gl*3+2] = r[2]; }
 }
 
+/* threads the parallel loops of this library run on (for the benchmark's "cores" field; no arithmetic) */
+int orc_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
 int orc_transport(const orc_grid* grid, const float* rho,
                   int32_t n_fields, const orc_field* fields, const orc_spot* spots,
                   int64_t n_segs, const orc_segment* segs,
@@ -198,23 +211,32 @@ int orc_transport(const orc_grid* grid, const float* rho,
     const double scale = ldexp(1.0, fixed_shift);
     if (probe_xy) for (int64_t i = 0; i < (int64_t)n_probe * hist_count * 2; ++i) probe_xy[i] = NAN;
     int64_t inc = 0, dep = 0, esc = 0; uint64_t steps = 0, hist = 0;
-    for (int64_t s = 0; s < n_segs; ++s) {
-        const orc_segment* sg = &segs[s];
-        if (sg->n_hist <= 0) continue;
+    /* Histories are independent (T1: one Philox stream each) and every tally is an integer sum, so the order in which
+     * they run changes nothing.  They are numbered 0 .. total-1 across the segments (begin[s] = histories of the
+     * segments before s) and handed to the threads from ONE parallel loop: a loop per segment left the threads idle
+     * on plans with thousands of segments of a few histories each. */
+    int64_t* begin = (int64_t*)malloc((size_t)(n_segs + 1) * sizeof(int64_t));
+    if (!begin) return -2;
+    begin[0] = 0;
+    for (int64_t s = 0; s < n_segs; ++s) begin[s + 1] = begin[s] + (segs[s].n_hist > 0 ? segs[s].n_hist : 0);
+    const int64_t total = begin[n_segs];
+    #pragma omp parallel for schedule(dynamic, 256) reduction(+:inc,dep,esc,steps,hist)
+    for (int64_t i = 0; i < total; ++i) {
+        int64_t lo = 0, hi = n_segs;                 /* the segment s with begin[s] <= i < begin[s + 1] */
+        while (hi - lo > 1) { int64_t mid = lo + (hi - lo) / 2; if (begin[mid] <= i) lo = mid; else hi = mid; }
+        const orc_segment* sg = &segs[lo];
         const orc_spot*  sp = &spots[sg->spot];
         const orc_field* F  = &fields[sg->field];
-        #pragma omp parallel for schedule(dynamic, 64) reduction(+:inc,dep,esc,steps,hist)
-        for (int64_t j = 0; j < sg->n_hist; ++j) {
-            uint64_t g = (uint64_t)(sg->first_history + j);
-            tally T = { 0, 0, 0, 0 };
-            int64_t gl = (int64_t)g - hist_base;
-            int traced = (probe_xy || stop_xyz) && gl >= 0 && gl < hist_count;
-            one_history(grid, rho, F, sp, sg->weight, seed, g, scale, flags, Q, &T,
-                        traced && probe_xy ? n_probe : 0, probe_faces, probe_xy, hist_count, gl,
-                        traced ? stop_xyz : 0);
-            inc += T.inc; dep += T.dep; esc += T.esc; steps += T.steps; hist += 1;
-        }
+        uint64_t g = (uint64_t)(sg->first_history + (i - begin[lo]));
+        tally T = { 0, 0, 0, 0 };
+        int64_t gl = (int64_t)g - hist_base;
+        int traced = (probe_xy || stop_xyz) && gl >= 0 && gl < hist_count;
+        one_history(grid, rho, F, sp, sg->weight, seed, g, scale, flags, Q, &T,
+                    traced && probe_xy ? n_probe : 0, probe_faces, probe_xy, hist_count, gl,
+                    traced ? stop_xyz : 0);
+        inc += T.inc; dep += T.dep; esc += T.esc; steps += T.steps; hist += 1;
     }
+    free(begin);
     if (stats) {
         stats->histories = hist; stats->steps = steps;
         stats->q_incident = inc; stats->q_deposited = dep; stats->q_escaped = esc;
