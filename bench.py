@@ -25,7 +25,7 @@ sys.path.insert(0, ROOT)
 # summary under profiles/ is missing -- the reported figure is the measured one (profile_metrics)
 OPS_PER_STEP_MODEL = 262
 # histories of the bounded oracle sample (10-30 s of host work on 16 cores); the reference arm uses half per step
-ORACLE_SAMPLE = {"config5": 200_000, "config3": 400_000, "config2": 200_000}
+ORACLE_SAMPLE = {"config5": 1_000_000, "config3": 2_000_000, "config2": 1_000_000}
 # per-kernel numbers taken from the committed ncu captures (kernel, workload, metric, value); written by hand from the
 # reports named in profiles/r2_summary.md
 PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernel_metrics.csv")
@@ -56,7 +56,46 @@ def parse():
                          "accumulation stress of BASELINE.json config 4 alone (push / DIM at n = 2, 4, 8 and (2,2,5))")
     ap.add_argument("--histories", type=int, default=0, help="override the config's history count (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dry-ranks", action="store_true",
+                    help="launch check without a GPU: start the ranks, count them over gloo, print {'dry': true, ...}")
     return ap.parse_args()
+
+
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(args):
+    """`python bench.py --gpus N` (N > 1) outside a launcher: start N ranks of this same command, one per GPU, through
+    torch.distributed.run on 127.0.0.1 (the line the driver uses) and hand back its exit code.  Rank 0 prints the one
+    JSON line.  Fails loudly when fewer than N devices are visible; NCCL's own logging is left as the caller set it."""
+    if not args.dry_ranks:
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def dry_ranks(args, rank, world):
+    """the launch path alone (CPU, gloo): every rank joins, the ranks are counted with an all-reduce, rank 0 prints"""
+    import torch
+    import torch.distributed as dist
+    seen = 1
+    if world > 1:
+        dist.init_process_group("gloo")
+        t = torch.ones(1, dtype=torch.int64)
+        dist.all_reduce(t)
+        seen = int(t[0])
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"dry": True, "n_gpus": world, "ranks_seen": seen, "requested": args.gpus}), flush=True)
 
 
 def make_workload(name, rank, histories=0):
@@ -322,11 +361,20 @@ def run_reference(args, rank, world):
 
 def main():
     args = parse()
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if args.impl == "reference":
+        run_reference(args, int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")))
+        return
+    if args.gpus > 1 and args.workload != "config4" and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_ranks(args))                             # plain `python bench.py --gpus N`: become N ranks
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
-        run_reference(args, rank, world)
+    if world != args.gpus and args.workload != "config4":
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s)")
+    if args.dry_ranks:
+        dry_ranks(args, rank, world)
         return
     if args.workload == "config4":
         if rank == 0:

@@ -1,6 +1,7 @@
-"""Host logic of bench.py's N > 1 path on CPU (gloo, world_size 2): replicas only -- every rank times an independent
-plan, times are reduced with MAX and histories with SUM; the reference arm runs on rank 0
-alone.  No GPU and no compute call is involved."""
+"""Host logic of bench.py's N > 1 path on CPU (gloo, world_size 2).  The N ranks share ONE plan (strong scaling: each
+transports its slice of every phase's histories); times are reduced with MAX and histories with
+SUM; `python bench.py --gpus N` outside a launcher starts the N ranks itself; the reference arm runs on rank 0 alone.
+No GPU and no compute call is involved."""
 import json
 import os
 import subprocess
@@ -46,3 +47,20 @@ def test_reference_arm_runs_on_rank0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_2_without_a_launcher_starts_two_ranks():
+    # what the driver's N = 1 style command line does for N > 1: no WORLD_SIZE in the environment
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-ranks"],
+                       env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert lines == [{"dry": True, "n_gpus": 2, "ranks_seen": 2, "requested": 2}]
+
+
+def test_rank_count_must_match_gpus():
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-ranks"],
+                       env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode != 0 and "--gpus 2" in r.stderr
