@@ -121,3 +121,48 @@ def test_eq2_sums_phases_in_double():
     want = (doses[0].astype(np.float64) + doses[1] + doses[2] + doses[3]).astype(np.float32)
     assert (out[:-1, :-1, :-1] == want[:-1, :-1, :-1]).all() and np.abs(out - want).max() < 1e-6
     assert st["subvoxels"] == 3 * 125
+
+
+@pytest.mark.parametrize("ns", [(2, 2, 2), (4, 2, 4)])
+@pytest.mark.parametrize("decades", [0, 30])
+def test_subvoxel_sum_order_is_a_free_choice(ns, decades):
+    # Reading D4: Eq. 3 is a plain mean and fixes no summation order; the oracle adds the subvoxels
+    # of a voxel in (b, a, c) order (z innermost; round 1 used (c, b, a)).  The choice must not matter beyond the
+    # rounding of a double sum.  The per-subvoxel values come from the oracle itself at n = 1 on the refined grid: with
+    # power-of-two spacings and subdivisions every subvoxel centre of R is, exactly, a voxel centre of the refined grid.
+    # decades = 0: doses of one magnitude -- a few fp32 values add up EXACTLY in double, so every order gives the same
+    # bits; decades = 30: doses spread over 30 decades, where the additions do round and the orders may part by ulps.
+    rng = np.random.default_rng(5)
+    shape = (6, 7, 8)
+    R = grid(shape, (2.0, 4.0, 2.0), (-1.0, 0.5, 2.0))
+    fine = grid((shape[0] * ns[2], shape[1] * ns[1], shape[2] * ns[0]), (2.0 / ns[0], 4.0 / ns[1], 2.0 / ns[2]),
+                (-1.0, 0.5, 2.0))
+    Dg = grid((5, 6, 7), (4.0, 8.0, 4.0), (-3.0, -4.0, -2.0))
+    S = grid((7, 8, 9), (2.0, 4.0, 2.0), (-2.0, -1.5, 1.0))
+    disp = smooth_field(rng, (5, 6, 7), 2.5)
+    dose = rng.uniform(0.5, 2.0, size=(7, 8, 9)) * 10.0 ** rng.uniform(-decades, 0, size=(7, 8, 9))
+    dose = dose.astype(np.float32)
+    got, st = orc.dim_pull(R, ns, Dg, disp, S, dose)
+    val, st1 = orc.dim_pull(fine, (1, 1, 1), Dg, disp, S, dose)            # one value per subvoxel (0 where dropped)
+    assert st1["subvoxels"] == st["subvoxels"] and st1["dropped_outside_ref"] == st["dropped_outside_ref"]
+    assert st1["dropped_outside_dvf"] == st["dropped_outside_dvf"] == 0
+    v = val.reshape(shape[0], ns[2], shape[1], ns[1], shape[2], ns[0])     # [k, c, j, b, i, a]
+    n3 = float(ns[0] * ns[1] * ns[2])
+
+    def summed(order):
+        s = np.zeros(shape, np.float64)
+        for idx in order:
+            s = s + v[:, idx["c"], :, idx["b"], :, idx["a"]]              # one double addition per subvoxel, in order
+        return s / n3
+
+    bac = [dict(b=b, a=a, c=c) for b in range(ns[1]) for a in range(ns[0]) for c in range(ns[2])]
+    cba = [dict(b=b, a=a, c=c) for c in range(ns[2]) for b in range(ns[1]) for a in range(ns[0])]
+    assert (summed(bac) == got).all()                                      # the order the oracle states, bit for bit
+    alt = summed(cba)                                                      # the order of round 1
+    if decades == 0:
+        assert (alt == got).all()
+    else:
+        assert np.abs(alt - got).max() > 0                                 # here the order does show ...
+    assert (np.abs(alt - got) <= 4 * np.spacing(np.abs(got))).all()        # ... by a few ulp of the double sum, no more
+    # far below what the fp32 output of Eq. 2 resolves
+    assert (alt.astype(np.float32) == got.astype(np.float32)).mean() > 0.999
