@@ -24,8 +24,12 @@ sys.path.insert(0, ROOT)
 # hand-count MODEL of the lane-operations of one condensed-history step; used only when the ncu
 # summary under profiles/ is missing -- the reported figure is the measured one (profile_metrics)
 OPS_PER_STEP_MODEL = 262
+# lane-instructions per step that ARE the algorithm (DESIGN.md section 5 census of the transport kernel's SASS: 199.1 for
+# the model of every lane + the voxel-change work of the lanes that change voxel); the rest of the executed count is
+# loop control, refill and source sampling.  Reported beside the issue utilisation as `frac_algorithmic`.
+ALGORITHM_OPS_PER_STEP = 210.0
 # histories of the bounded oracle sample (10-30 s of host work on 16 cores); the reference arm uses half per step
-ORACLE_SAMPLE = {"config5": 1_000_000, "config3": 2_000_000, "config2": 1_000_000}
+ORACLE_SAMPLE = {"config5": 2_000_000, "config3": 4_000_000, "config2": 2_000_000}
 # per-kernel numbers taken from the committed ncu captures (kernel, workload, metric, value); written by hand from the
 # reports named in profiles/r2_summary.md
 PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernel_metrics.csv")
@@ -42,6 +46,30 @@ def profile_metrics():
                     out[(c[0], c[1], c[2])] = float(c[3])
     except OSError:
         pass
+    return out
+
+
+def profile_source_state():
+    """{kernel: "current" | "STALE: ..."} -- the `#source,kernel,path,hash` stamps of the metrics file (git blob hash
+    of the kernel's source when it was captured) against the same hash of the file in the working tree"""
+    import hashlib
+    out = {}
+    try:
+        with open(PROFILE_CSV) as f:
+            stamps = [line.strip().split(",") for line in f if line.startswith("#source,")]
+    except OSError:
+        return out
+    for c in stamps:
+        if len(c) < 4:
+            continue
+        kernel, path, want = c[1], c[2], c[3]
+        try:
+            data = open(os.path.join(ROOT, path), "rb").read()
+            have = hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+        except OSError:
+            have = "missing"
+        out[kernel] = "current" if have == want else \
+            f"STALE: {path} is {have[:10]}, the capture was taken of {want[:10]} -- re-capture and re-stamp"
     return out
 
 
@@ -238,8 +266,12 @@ def run_accumulation_stress(args):
     peaks, peak_kind = measured_peaks()
     prof = profile_metrics()
     props = torch.cuda.get_device_properties(0)
-    issue_peak = props.multi_processor_count * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-    warm, steps = max(args.warmup, 1) if args.warmup != 3 else 1, args.steps if args.steps != 3 else 2
+    # defaults long enough for the NVML sampler (one sample per 0.1 s) to see the clocks under load
+    warm, steps = max(args.warmup, 1) if args.warmup != 3 else 2, args.steps if args.steps != 3 else 20
+    src_state = profile_source_state()
+    for _ in range(warm):                                            # clocks up before the sampler starts
+        ctx.accumulate_subvoxel(c["ref_phase"], (4, 4, 4), doses)
+    sampler = ClockSampler(0); sampler.start()
 
     def timed(fn, ns):
         ms = fin = 0.0
@@ -252,9 +284,22 @@ def run_accumulation_stress(args):
     out = {"metric": "subvoxels/s (accumulation stress)", "unit": "subvoxels/s", "n_gpus": 1, "steps": steps,
            "warmup": warm, "higher_is_better": True, "dtype": "f32+i64", "data": "synthetic",
            "config": {"workload": "config4", "grid": list(c["doses"].shape[1:]), "source_phases": n_src},
-           "peaks": {"hbm_GBps": peaks["hbm_gbs"], "issue_Tlaneops": issue_peak, "kind": peak_kind}, "push": {}, "dim": {}}
+           "push": {}, "dim": {}}
+    raw = {"push": {}, "dim": {}}
     for ns in [(2, 2, 2), (4, 4, 4), (8, 8, 8), (2, 2, 5)]:
-        ms, fin, st = timed(ctx.accumulate_subvoxel, ns)
+        raw["push"][ns] = timed(ctx.accumulate_subvoxel, ns)
+    for ns in [(1, 1, 1), (2, 2, 2), (4, 4, 4), (8, 8, 8)]:
+        raw["dim"][ns] = timed(ctx.accumulate_dim, ns)
+    torch.cuda.synchronize()
+    clocks = sampler.summary()
+    sm_mhz = clocks["sm_mhz"] or peaks.get("sm_max_mhz", 1965.0)
+    issue_peak = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
+    out["clocks"] = clocks
+    out["peaks"] = {"hbm_GBps": peaks["hbm_gbs"], "issue_Tlaneops": issue_peak, "kind": peak_kind,
+                    "issue_how": f"SMs x 128 lanes x median SM clock under load ({sm_mhz:.0f} MHz)"}
+    out["lane_ops_source"] = {k: src_state.get(k, "unstamped") for k in ("emtm_push_kernel", "dim_pull_kernel")}
+    for ns in [(2, 2, 2), (4, 4, 4), (8, 8, 8), (2, 2, 5)]:
+        ms, fin, st = raw["push"][ns]
         key = "x".join(map(str, ns))
         ops = prof.get(("emtm_push_kernel", f"config4_{key}", "thread_inst_per_subvoxel"))
         rate = st["subvoxels"] / (ms * 1e-3)
@@ -263,7 +308,7 @@ def run_accumulation_stress(args):
                             "lane_ops_per_subvoxel": ops, "issue_frac": None if not ops else rate * ops / 1e12 / issue_peak,
                             "finalize_ms": fin, "finalize_GBps": nvox * (16 * n_src + 8) / (fin * 1e-3) / 1e9}
     for ns in [(1, 1, 1), (2, 2, 2), (4, 4, 4), (8, 8, 8)]:
-        ms, fin, st = timed(ctx.accumulate_dim, ns)
+        ms, fin, st = raw["dim"][ns]
         key = "x".join(map(str, ns))
         ops = prof.get(("dim_pull_kernel", f"config4_{key}", "thread_inst_per_subvoxel"))
         rate = st["subvoxels"] / (ms * 1e-3)
@@ -493,11 +538,15 @@ def main():
     peak = world * props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e12
     # lane-instructions per condensed-history step: executed thread instructions of the transport kernel / steps, from
     # the committed ncu capture of the kernel (profiles/); the hand-count model only when that file is missing
-    ops_step = prof.get(("transport_kernel", wl, "thread_inst_per_step")) or \
-        prof.get(("transport_kernel", "config5", "thread_inst_per_step"))
-    ops_kind = "ncu smsp__thread_inst_executed / steps (profiles/r2_kernel_metrics.csv)"
+    # (a count captured on another workload is not borrowed: the voxel-change share of a step depends on the geometry)
+    src_state = profile_source_state()
+    ops_step = prof.get(("transport_kernel", wl, "thread_inst_per_step"))
+    ops_kind = "ncu smsp__thread_inst_executed / steps (profiles/r2_kernel_metrics.csv), source " + \
+        src_state.get("transport_kernel", "unstamped")
+    if src_state.get("transport_kernel", "").startswith("STALE"):
+        ops_kind = src_state["transport_kernel"]
     if not ops_step:
-        ops_step, ops_kind = OPS_PER_STEP_MODEL, "hand-count model (no ncu capture found)"
+        ops_step, ops_kind = OPS_PER_STEP_MODEL, f"hand-count model (no ncu capture of the transport kernel on {wl})"
     achieved = steps_per_s * ops_step / 1e12
     acc_bytes = stats["n_src"] * nvox * (20 + 16)
     fin_bytes = nvox * (16 * len(stats["src"]) + 8)
@@ -525,6 +574,10 @@ def main():
         "transport_histories_per_s": hist / (tr_ms * 1e-3),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
+                     "frac_kind": "issue utilisation: EXECUTED lane-instructions (algorithm + loop/refill overhead) over the "
+                                  "lane-issue peak",
+                     "frac_algorithmic": steps_per_s * ALGORITHM_OPS_PER_STEP / 1e12 / peak,
+                     "algorithmic_lane_ops_per_step": ALGORITHM_OPS_PER_STEP,
                      "traffic": prof.get(("transport_kernel", wl, "dram_bytes_per_launch")), "kernel": "transport_kernel",
                      "lane_ops_per_step": ops_step, "lane_ops_source": ops_kind,
                      "how": f"{ops_step:.1f} executed lane-instructions per step x {steps_per_s:.3e} steps/s over the CUDA-event time of the "
@@ -545,6 +598,7 @@ def main():
                                  "unit": "Tlane-op/s", "frac": stats["subvoxels"] / push_s * push_ops / 1e12 / push_peak,
                                  "lane_ops_per_subvoxel": push_ops},
                                 "binding": "alu" if push_ops else "unknown (no ncu capture for this subdivision)",
+                                "lane_ops_source": src_state.get("emtm_push_kernel", "unstamped"),
                                 "measured_hbm_copy": probes["hbm_copy"] / 1e9,
                                 "subvoxels_per_s": stats["subvoxels"] / push_s,
                                 "finalize_GBps": fin_bytes / (stats["finalize_ms"] * 1e-3) / 1e9,

@@ -64,3 +64,25 @@ def test_rank_count_must_match_gpus():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-ranks"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode != 0 and "--gpus 2" in r.stderr
+
+
+def test_roofline_figures_are_tied_to_the_kernel_source(tmp_path, monkeypatch):
+    # the lane-instruction counts bench.py multiplies with come from ncu captures under profiles/; the metrics file
+    # carries the git blob hash of each kernel's source at capture time, and an edited source must show as STALE
+    import hashlib
+    sys.path.insert(0, ROOT)
+    import bench
+    src = tmp_path / "kernel.cu"
+    src.write_text("__global__ void k() {}\n")
+    data = src.read_bytes()
+    blob = hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+    git = subprocess.run(["git", "hash-object", str(src)], capture_output=True, text=True).stdout.strip()
+    assert not git or git == blob                                          # the same hash `git hash-object` prints
+    csv = tmp_path / "metrics.csv"
+    csv.write_text(f"# header\n#source,transport_kernel,{src},{blob}\nkernel,workload,metric,value,source\n"
+                   "transport_kernel,config5,thread_inst_per_step,217.89,x.ncu-rep\n")
+    monkeypatch.setattr(bench, "PROFILE_CSV", str(csv))
+    assert bench.profile_source_state() == {"transport_kernel": "current"}
+    assert bench.profile_metrics()[("transport_kernel", "config5", "thread_inst_per_step")] == 217.89
+    src.write_text("__global__ void k() {}  // a comment\n")
+    assert bench.profile_source_state()["transport_kernel"].startswith("STALE")
