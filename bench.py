@@ -32,11 +32,11 @@ ALGORITHM_OPS_PER_STEP = 210.0
 ORACLE_SAMPLE = {"config5": 2_000_000, "config3": 4_000_000, "config2": 2_000_000}
 # per-kernel numbers taken from the committed ncu captures (kernel, workload, metric, value); written by hand from the
 # reports named in profiles/r2_summary.md
-PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernel_metrics.csv")
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r3_kernel_metrics.csv")
 
 
 def profile_metrics():
-    """{(kernel, workload, metric): value} from profiles/r2_kernel_metrics.csv; {} if the file is absent"""
+    """{(kernel, workload, metric): value} from profiles/r3_kernel_metrics.csv; {} if the file is absent"""
     out = {}
     try:
         with open(PROFILE_CSV) as f:
@@ -541,7 +541,7 @@ def main():
     # (a count captured on another workload is not borrowed: the voxel-change share of a step depends on the geometry)
     src_state = profile_source_state()
     ops_step = prof.get(("transport_kernel", wl, "thread_inst_per_step"))
-    ops_kind = "ncu smsp__thread_inst_executed / steps (profiles/r2_kernel_metrics.csv), source " + \
+    ops_kind = "ncu smsp__thread_inst_executed / steps (profiles/r3_kernel_metrics.csv), source " + \
         src_state.get("transport_kernel", "unstamped")
     if src_state.get("transport_kernel", "").startswith("STALE"):
         ops_kind = src_state["transport_kernel"]
@@ -572,6 +572,7 @@ def main():
         "gpu_launches": launches,
         "kernel_ms_per_step": {"transport": tr_ms / args.steps, "push": stats["push_ms"], "acc_finalize": stats["finalize_ms"]},
         "transport_histories_per_s": hist / (tr_ms * 1e-3),
+        "mc_steps_per_plan": mc_steps / args.steps,
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
                      "frac_kind": "issue utilisation: EXECUTED lane-instructions (algorithm + loop/refill overhead) over the "

@@ -96,13 +96,15 @@ typedef struct {
 #define PBS4D_NO_STRAGGLE  2u      /* source energy spread / spot size                                      */
 #define PBS4D_NO_ESPREAD   4u
 #define PBS4D_NO_SPOTSIZE  8u
+#define PBS4D_TEST_STEP_CAP_64 16u /* test switch: the transport's step cap (hang guard) at 64 steps instead of 2^20 */
 
 typedef struct {
     uint64_t histories, steps;
     int64_t  q_incident, q_deposited, q_escaped;        /* fixed point, quantum 2^-fixed_shift MeV */
     int32_t  fixed_shift; int32_t pad;
     float    kernel_ms;                                 /* device time of the transport kernel (CUDA events) */
-    int32_t  pad2;
+    int32_t  aborted;                                   /* histories stopped by the step cap (2^20 steps; their energy
+                                                           is deposited where they stood): 0 for any valid input */
     uint64_t scoring_atomics;                           /* red.global.add.u64 issued by the scoring (one per voxel visit) */
 } pbs4d_mc_stats;
 

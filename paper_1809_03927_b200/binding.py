@@ -26,7 +26,7 @@ SEG_DT = np.dtype([("field", "i4"), ("phase", "i4"), ("spot", "i4"), ("pad", "i4
 DICOM_DVF_DT = np.dtype([("nx", "i4"), ("ny", "i4"), ("nz", "i4"), ("pad", "i4"), ("start", "f8", 3), ("delta", "f8", 3),
                          ("row_cos", "f8", 3), ("col_cos", "f8", 3), ("pre", "f8", 16), ("post", "f8", 16)])
 
-NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE = 1, 2, 4, 8
+NO_MCS, NO_STRAGGLE, NO_ESPREAD, NO_SPOTSIZE, TEST_STEP_CAP_64 = 1, 2, 4, 8, 16
 
 EXPORTS = ["pbs4d_create", "pbs4d_destroy", "pbs4d_last_error", "pbs4d_set_ct_phases", "pbs4d_set_density_phases",
            "pbs4d_set_dvf", "pbs4d_set_plan_spots", "pbs4d_set_mc_flags", "pbs4d_simulate_delivery",
@@ -82,7 +82,7 @@ class TrialResult(C.Structure):
 class McStats(C.Structure):
     _fields_ = [("histories", C.c_uint64), ("steps", C.c_uint64), ("q_incident", C.c_int64),
                 ("q_deposited", C.c_int64), ("q_escaped", C.c_int64), ("fixed_shift", C.c_int32), ("pad", C.c_int32),
-                ("kernel_ms", C.c_float), ("pad2", C.c_int32), ("scoring_atomics", C.c_uint64)]
+                ("kernel_ms", C.c_float), ("aborted", C.c_int32), ("scoring_atomics", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_ if not n.startswith("pad")}

@@ -4,6 +4,7 @@
 #include "internal.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
 #include <algorithm>
 #include <chrono>
@@ -144,6 +145,16 @@ int on_exception(pbs4d_ctx* c) noexcept
 
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
 
+// One NVTX range per API call (tracing): a timeline or launch list taken with Nsight tools shows
+// which pbs4d_* call every kernel and copy belongs to (the paper reports its times per component, PAPER.md:187-195
+// Table II).  Header-only NVTX 3: without a tool attached a push / pop is a load and a branch.
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+    NvtxRange(const NvtxRange&) = delete;
+    NvtxRange& operator=(const NvtxRange&) = delete;
+};
+
 // nullptr for a usable grid, else what is wrong with it.  The per-axis limits are those of the launch geometry: the
 // accumulation kernels put ceil(ny / 4) CTAs on grid.y and ceil(nz / 4) on grid.z, the resampling density kernel nz on
 // grid.z (each at most 65535), and rows (ny * nz) go on grid.x, which the total bounds.
@@ -190,6 +201,7 @@ extern "C" {
 
 int pbs4d_create(pbs4d_ctx** out, int device, void* cuda_stream) try
 {
+    const NvtxRange nvtx_range_("pbs4d_create");
     if (!out) return PBS4D_ERR_ARG;
     *out = nullptr;
     int n_dev = 0;
@@ -235,6 +247,7 @@ const char* pbs4d_last_error(const pbs4d_ctx* ctx) { return ctx ? ctx->err.c_str
 int pbs4d_set_ct_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* ct, const int16_t* const* hu_dev,
                         const pbs4d_grid* dose_grid, int32_t n_pts, const float* hu_pts, const float* rho_pts) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_ct_phases");
     if (!ctx) return PBS4D_ERR_ARG;
     if (const char* why = grid_defect(ct)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_ct_phases: ct: ") + why);
     if (dose_grid) if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_ct_phases: dose_grid: ") + why);
@@ -269,6 +282,7 @@ catch (...) { return on_exception(ctx); }
 int pbs4d_set_density_phases(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d_grid* dose_grid,
                              const float* const* rho_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_density_phases");
     if (!ctx) return PBS4D_ERR_ARG;
     if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("set_density_phases: ") + why);
     if (n_phases < 1 || n_phases > 32 || !rho_dev)
@@ -320,6 +334,7 @@ static int store_dvf(pbs4d_ctx* ctx, std::vector<pbs4d_ctx::Dvf>& table, const c
 int pbs4d_set_dvf(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
                   const float* disp_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_dvf");
     if (!ctx) return PBS4D_ERR_ARG;
     return store_dvf(ctx, ctx->dvf, "set_dvf", src_phase, ref_phase, dvf_grid, disp_dev);
 }
@@ -328,6 +343,7 @@ catch (...) { return on_exception(ctx); }
 int pbs4d_set_dvf_pull(pbs4d_ctx* ctx, int32_t src_phase, int32_t ref_phase, const pbs4d_grid* dvf_grid,
                        const float* disp_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_dvf_pull");
     if (!ctx) return PBS4D_ERR_ARG;
     return store_dvf(ctx, ctx->dvf_pull, "set_dvf_pull", src_phase, ref_phase, dvf_grid, disp_dev);
 }
@@ -336,6 +352,7 @@ catch (...) { return on_exception(ctx); }
 int pbs4d_set_plan_spots(pbs4d_ctx* ctx, int32_t n_fields, const pbs4d_field* fields,
                          int64_t n_spots, const pbs4d_spot* spots) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_plan_spots");
     if (!ctx) return PBS4D_ERR_ARG;
     if (n_fields < 1 || !fields || n_spots < 1 || !spots) return fail(ctx, PBS4D_ERR_ARG, "set_plan_spots: bad argument");
     for (int64_t s = 0; s < n_spots; ++s) {
@@ -359,6 +376,7 @@ catch (...) { return on_exception(ctx); }
 
 int pbs4d_set_mc_flags(pbs4d_ctx* ctx, uint32_t flags) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_mc_flags");
     if (!ctx) return PBS4D_ERR_ARG;
     ctx->mc_flags = flags;
     return PBS4D_OK;
@@ -377,6 +395,7 @@ extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_
 extern "C" int pbs4d_simulate_delivery(pbs4d_ctx* ctx, const pbs4d_delivery_params* prm, uint64_t total_histories,
                                        pbs4d_phase_lists* out) try
 {
+    const NvtxRange nvtx_range_("pbs4d_simulate_delivery");
     return pbs4d_simulate_delivery_ext(ctx, prm, nullptr, total_histories, out, nullptr);
 }
 catch (...) { return on_exception(ctx); }
@@ -386,6 +405,7 @@ extern "C" int pbs4d_simulate_delivery_ext(pbs4d_ctx* ctx, const pbs4d_delivery_
                                            const pbs4d_delivery_ext* ext, uint64_t total_histories,
                                            pbs4d_phase_lists* out, int64_t* n_fills) try
 {
+    const NvtxRange nvtx_range_("pbs4d_simulate_delivery_ext");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery: null parameters");
     if (ctx->fields.empty()) return fail(ctx, PBS4D_ERR_ORDER, "simulate_delivery: call set_plan_spots first");
@@ -477,6 +497,7 @@ int upload_segments(pbs4d_ctx* ctx, int phase, cudaStream_t st)
 extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* phases, uint64_t seed, double per_protons,
                                     pbs4d_mc_stats* stats, float* elapsed_ms) try
 {
+    const NvtxRange nvtx_range_("pbs4d_mc_dose_phases");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: no densities (set_ct_phases)");
     if (!ctx->have_delivery) return fail(ctx, PBS4D_ERR_ORDER, "mc_dose_phases: call simulate_delivery first");
@@ -561,7 +582,8 @@ extern "C" int pbs4d_mc_dose_phases(pbs4d_ctx* ctx, int32_t n, const int32_t* ph
             pbs4d_mc_stats& s = stats[a];
             s.histories = tc[a].histories; s.steps = tc[a].steps;
             s.q_incident = tc[a].q_incident; s.q_deposited = tc[a].q_deposited; s.q_escaped = tc[a].q_escaped;
-            s.fixed_shift = ctx->fixed_shift; s.pad = 0; s.pad2 = 0; s.scoring_atomics = tc[a].reds;
+            s.fixed_shift = ctx->fixed_shift; s.pad = 0; s.scoring_atomics = tc[a].reds;
+            s.aborted = (int32_t)std::min<unsigned long long>(tc[a].aborted, 0x7fffffffull);
             s.kernel_ms = 0.0f;
             cudaEventElapsedTime(&s.kernel_ms, ev[2 * a], ev[2 * a + 1]);
         }
@@ -575,6 +597,7 @@ catch (...) { return on_exception(ctx); }
 extern "C" int pbs4d_mc_dose_phase(pbs4d_ctx* ctx, int32_t phase, uint64_t seed, double per_protons,
                                    float* dose_dev, float* rho_dev, pbs4d_mc_stats* stats) try
 {
+    const NvtxRange nvtx_range_("pbs4d_mc_dose_phase");
     if (!ctx) return PBS4D_ERR_ARG;
     const int rc = pbs4d_mc_dose_phases(ctx, 1, &phase, seed, per_protons, stats, nullptr);
     if (rc != PBS4D_OK) return rc;
@@ -588,6 +611,7 @@ catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_get_phase_energy(pbs4d_ctx* ctx, int32_t phase, int64_t* q_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_get_phase_energy");
     if (!ctx) return PBS4D_ERR_ARG;
     if (phase < 0 || phase >= ctx->n_phases || !q_dev) return fail(ctx, PBS4D_ERR_ARG, "get_phase_energy: bad argument");
     if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "get_phase_energy: mc_dose_phase not run for this phase");
@@ -614,6 +638,7 @@ extern "C" int pbs4d_shard_window(int64_t n_hist, int32_t rank, int32_t world, i
 
 extern "C" int pbs4d_set_shard(pbs4d_ctx* ctx, int32_t rank, int32_t world) try
 {
+    const NvtxRange nvtx_range_("pbs4d_set_shard");
     if (!ctx) return PBS4D_ERR_ARG;
     if (world < 1 || rank < 0 || rank >= world) return fail(ctx, PBS4D_ERR_ARG, "set_shard: need 0 <= rank < world");
     ctx->shard_rank = rank; ctx->shard_world = world;      // affects the mc_dose_phase(s) calls that follow only
@@ -623,6 +648,7 @@ catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_phase_energy_ptr(pbs4d_ctx* ctx, int32_t phase, int64_t** q_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_phase_energy_ptr");
     if (!ctx) return PBS4D_ERR_ARG;
     if (phase < 0 || phase >= ctx->n_phases || !q_dev) return fail(ctx, PBS4D_ERR_ARG, "phase_energy_ptr: bad argument");
     if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "phase_energy_ptr: mc_dose_phase not run for this phase");
@@ -633,6 +659,7 @@ catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_finalize_phase_dose(pbs4d_ctx* ctx, int32_t phase, double per_protons) try
 {
+    const NvtxRange nvtx_range_("pbs4d_finalize_phase_dose");
     if (!ctx) return PBS4D_ERR_ARG;
     if (phase < 0 || phase >= ctx->n_phases) return fail(ctx, PBS4D_ERR_ARG, "finalize_phase_dose: bad argument");
     if (!ctx->have_dose[phase]) return fail(ctx, PBS4D_ERR_ORDER, "finalize_phase_dose: mc_dose_phase not run for this phase");
@@ -731,6 +758,7 @@ extern "C" int pbs4d_accumulate_subvoxel(pbs4d_ctx* ctx, int32_t ref_phase, int3
                                          const float* const* phase_dose_dev, float* dose4d_dev,
                                          pbs4d_acc_stats* stats) try
 {
+    const NvtxRange nvtx_range_("pbs4d_accumulate_subvoxel");
     if (!ctx) return PBS4D_ERR_ARG;
     return accumulate_impl(ctx, "accumulate_subvoxel", ref_phase, nsx, nsy, nsz, phase_dose_dev, 0xFFFFFFFFu, true, true,
                            dose4d_dev, stats);
@@ -742,6 +770,7 @@ catch (...) { return on_exception(ctx); }
 extern "C" int pbs4d_accumulate_push(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
                                      const float* const* phase_dose_dev, uint32_t src_mask, pbs4d_acc_stats* stats) try
 {
+    const NvtxRange nvtx_range_("pbs4d_accumulate_push");
     if (!ctx) return PBS4D_ERR_ARG;
     return accumulate_impl(ctx, "accumulate_push", ref_phase, nsx, nsy, nsz, phase_dose_dev, src_mask, true, false,
                            nullptr, stats);
@@ -751,6 +780,7 @@ catch (...) { return on_exception(ctx); }
 extern "C" int pbs4d_accumulate_finalize(pbs4d_ctx* ctx, int32_t ref_phase, const float* const* phase_dose_dev,
                                          float* dose4d_dev, pbs4d_acc_stats* stats) try
 {
+    const NvtxRange nvtx_range_("pbs4d_accumulate_finalize");
     if (!ctx) return PBS4D_ERR_ARG;
     return accumulate_impl(ctx, "accumulate_finalize", ref_phase, 1, 1, 1, phase_dose_dev, 0u, false, true, dose4d_dev,
                            stats);
@@ -759,6 +789,7 @@ catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_accumulator_ptrs(pbs4d_ctx* ctx, int32_t src_phase, int64_t** e_dev, int64_t** m_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_accumulator_ptrs");
     if (!ctx) return PBS4D_ERR_ARG;
     if (src_phase < 0 || src_phase >= ctx->n_phases || !e_dev || !m_dev)
         return fail(ctx, PBS4D_ERR_ARG, "accumulator_ptrs: bad argument");
@@ -770,6 +801,7 @@ catch (...) { return on_exception(ctx); }
 
 extern "C" int pbs4d_get_accumulators(pbs4d_ctx* ctx, int32_t src_phase, int64_t* e_dev, int64_t* m_dev) try
 {
+    const NvtxRange nvtx_range_("pbs4d_get_accumulators");
     if (!ctx) return PBS4D_ERR_ARG;
     if (src_phase < 0 || src_phase >= ctx->n_phases || !e_dev || !m_dev)
         return fail(ctx, PBS4D_ERR_ARG, "get_accumulators: bad argument");
@@ -789,6 +821,7 @@ extern "C" int pbs4d_simulate_delivery_trial(pbs4d_ctx* ctx, const pbs4d_trial_s
                                              const pbs4d_delivery_params* prm, const pbs4d_delivery_ext* ext,
                                              uint64_t total_histories, pbs4d_phase_lists* out, int64_t* n_fills) try
 {
+    const NvtxRange nvtx_range_("pbs4d_simulate_delivery_trial");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!spec || !prm) return fail(ctx, PBS4D_ERR_ARG, "simulate_delivery_trial: null argument");
     if (ctx->fields.empty()) return fail(ctx, PBS4D_ERR_ORDER, "simulate_delivery_trial: call set_plan_spots first");
@@ -817,6 +850,7 @@ extern "C" int pbs4d_run_trials(pbs4d_ctx* ctx, const pbs4d_trial_spec* spec, in
                                 uint64_t total_histories, uint64_t seed, int32_t ref_phase, int32_t nsx, int32_t nsy,
                                 int32_t nsz, float* const* dose4d_dev, pbs4d_trial_result* results) try
 {
+    const NvtxRange nvtx_range_("pbs4d_run_trials");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!spec || !prm || !dose4d_dev || first < 0 || count < 1 || first + count > spec->n_trials)
         return fail(ctx, PBS4D_ERR_ARG, "run_trials: bad argument");
@@ -866,6 +900,7 @@ extern "C" int pbs4d_run_plan_host(pbs4d_ctx* ctx, int32_t n_phases, const pbs4d
                                    int32_t nsx, int32_t nsy, int32_t nsz, float* dose4d_host, uint64_t* histories_run,
                                    uint64_t* h2d_bytes, double* seconds) try
 {
+    const NvtxRange nvtx_range_("pbs4d_run_plan_host");
     if (!ctx) return PBS4D_ERR_ARG;
     if (const char* why = grid_defect(ct)) return fail(ctx, PBS4D_ERR_ARG, std::string("run_plan_host: ct: ") + why);
     if (dose_grid) if (const char* why = grid_defect(dose_grid)) return fail(ctx, PBS4D_ERR_ARG, std::string("run_plan_host: dose_grid: ") + why);
@@ -1008,6 +1043,7 @@ catch (...) { return on_exception(ctx); }
 // ------------------------------------------------------------------------------------------------------------------
 extern "C" int pbs4d_roofline_probe(pbs4d_ctx* ctx, int32_t kind, double* value) try
 {
+    const NvtxRange nvtx_range_("pbs4d_roofline_probe");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!value || kind < PBS4D_PROBE_FP32_ISSUE || kind > PBS4D_PROBE_HBM_COPY)
         return fail(ctx, PBS4D_ERR_ARG, "roofline_probe: bad argument");
@@ -1029,6 +1065,7 @@ catch (...) { return on_exception(ctx); }
 extern "C" int pbs4d_accumulate_dim(pbs4d_ctx* ctx, int32_t ref_phase, int32_t nsx, int32_t nsy, int32_t nsz,
                                     const float* const* phase_dose_dev, float* dose4d_dev, pbs4d_acc_stats* stats) try
 {
+    const NvtxRange nvtx_range_("pbs4d_accumulate_dim");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!ctx->have_density) return fail(ctx, PBS4D_ERR_ORDER, "accumulate_dim: no grid (set_ct_phases/set_density_phases)");
     if (ref_phase < 0 || ref_phase >= ctx->n_phases || nsx < 1 || nsy < 1 || nsz < 1 || nsx > 64 || nsy > 64 ||
@@ -1084,6 +1121,7 @@ catch (...) { return on_exception(ctx); }
 extern "C" int pbs4d_build_dvf(pbs4d_ctx* ctx, const pbs4d_dicom_dvf* info, const float* delta_dev, float* rf_dev,
                                float* disp_dev, pbs4d_grid* grid_out) try
 {
+    const NvtxRange nvtx_range_("pbs4d_build_dvf");
     if (!ctx) return PBS4D_ERR_ARG;
     if (!info || !delta_dev || (!rf_dev && !disp_dev) || info->nx < 1 || info->ny < 1 || info->nz < 1 ||
         (double)info->nx * info->ny * info->nz >= 2.0e9 || !(info->delta[0] > 0.0) || !(info->delta[1] > 0.0) ||

@@ -45,6 +45,7 @@ struct TransportCounters {       // device tallies of one launch (zeroed before 
     long long q_incident, q_deposited, q_escaped;
     unsigned long long next_history;      // work counter: next local history index to hand out
     unsigned long long reds;              // scoring atomics issued
+    unsigned long long aborted;           // histories stopped by the step cap (hang guard)
 };
 
 // Launchers (all asynchronous on `st`).

@@ -17,7 +17,7 @@
 //    the values at the midpoint energy are read off the same pair of nodes (one lookup per step);
 //  * one reciprocal per step for the voxel-face distance (the nearest face is found by cross-multiplication),
 //    1/density cached per voxel visit, Gaussian factors folded under one square root each, small-angle polynomial
-//    for the polar deflection, uniform floats built with bit operations: 9 MUFU per step instead of ~27;
+//    for the polar deflection, uniform floats built with bit operations: 10 MUFU per step instead of ~27;
 //  * Philox round keys are kernel parameters (constant bank operands);
 //  * position is voxel-local (0 <= p <= h) so face distances keep full fp32 resolution;
 //  * deposits are converted to int64 quanta of 2^-k MeV and summed in a register while the history stays in one
@@ -51,6 +51,7 @@ struct Params {
     int32_t n_segs;
     long long hist_begin, n_hist;             // this launch transports local histories hist_begin .. hist_begin + n_hist - 1
     uint32_t flags;
+    uint32_t max_steps;                       // hang guard: a history that reaches this many steps is absorbed where it is
     uint32_t k0[10], k1[10];                  // Philox round keys
     unsigned long long* Q;
     TransportCounters* counters;
@@ -259,12 +260,12 @@ __global__ void __launch_bounds__(kThreads, 4)
 transport_kernel(const __grid_constant__ Params P)
 {
     __shared__ float4 s_tab[kTabNodes];
-    __shared__ long long s_tally[6];
+    __shared__ long long s_tally[7];                    // [6]: histories stopped by the step cap
     __shared__ uint32_t s_pool[kWarps][kPoolWords][32];
     for (int i = threadIdx.x; i < kTabNodes; i += kThreads) s_tab[i] = P.tab[i];
     unsigned tab_addr;                                  // laundered through asm: kept in a register, not rebuilt per step
     asm volatile("mov.u32 %0, %1;" : "=r"(tab_addr) : "r"((unsigned)__cvta_generic_to_shared(s_tab)));
-    if (threadIdx.x < 6) s_tally[threadIdx.x] = 0;
+    if (threadIdx.x < 7) s_tally[threadIdx.x] = 0;
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u;
@@ -392,17 +393,15 @@ transport_kernel(const __grid_constant__ Params P)
 
             // T7: midpoint-rule mean loss
             const float t   = dens * s;                                       // g/cm2 (dens = 0.1 rho)
-            // E_m = E - S(E) t / 2 lies at most a few table intervals below E (an interval is 0.4-0.8 % of E, the
-            // half-step loss <= ~0.7 % of E in water-like media): S, V, T at E_m are read off the SAME pair of nodes,
-            // extrapolating linearly below the interval (error <= p(p-1)/2 (dE/E)^2 ~ 4e-5); only a half-step loss
-            // of more than 4 intervals (very dense voxels) takes a second table lookup
+            // E_m = E - S(E) t / 2 lies at most about one and a half table intervals below E, in ANY medium: the step
+            // is at most 2 % of the range at the voxel's density, so t <= 0.02 R_w(E) [g/cm2] whatever rho is, and with
+            // S R_w ~ E / p (p ~ 1.77) the half-step loss is <= 0.01 E / p ~ 0.6 % of E, an interval being 0.4-0.8 % of
+            // E.  S, V, T at E_m are therefore read off the SAME pair of nodes, extrapolating linearly below the
+            // interval (error <= p(p-1)/2 (dE/E)^2 ~ 4e-5).  (Until round 3 a second lookup stood here for losses of
+            // more than 4 intervals; the bound shows it could not be reached, and no test ever took it.)
             const float half = fminf(0.5f * S0 * t, L.E - 0.25f);
-            float  fm = fmaf(-half, k0.inv_w, k0.f);
-            float4 Am = A0, Bm = B0;
-            if (k0.f - fm > 4.0f) {
-                const Lookup km = locate(L.E - half);
-                Am = lds_node(tab_addr + (unsigned)km.i * 16u); Bm = lds_node(tab_addr + (unsigned)km.i * 16u + 16u); fm = km.f;
-            }
+            const float  fm = fmaf(-half, k0.inv_w, k0.f);
+            const float4 Am = A0, Bm = B0;
             const float Sm  = fmaf(fm, Bm.y - Am.y, Am.y);
             const float dEm = Sm * t;
 
@@ -425,7 +424,11 @@ transport_kernel(const __grid_constant__ Params P)
                 dE = fmaf(fast_sqrt(varg), -__cosf(a3), dEm);
             }
             dE = fminf(fmaxf(dE, 0.0f), L.E);
-            if (L.E - dE <= kEcut) { dE = L.E; alive = false; }
+            // below the cutoff the rest is deposited on the spot (T10).  The same exit serves as the hang guard of this
+            // persistent kernel: a history that has taken P.max_steps steps (2^20; a 250 MeV proton in air-filled
+            // lung needs a few thousand) is absorbed where it stands and counted in `aborted` -- never expected with
+            // inputs that passed validation, but a history that cannot end would otherwise hold the GPU for ever
+            if (L.E - dE <= kEcut || L.m >= P.max_steps) { dE = L.E; alive = false; }
 
             // T9/T11: score into the voxel the step lay in (register accumulation, flushed on voxel change)
             L.pend += __float2ll_rn(dE * L.wq);
@@ -479,7 +482,10 @@ transport_kernel(const __grid_constant__ Params P)
 
             if (crossing || !alive) {
                 flush(P, L, q_dep, n_red);
-                if (!alive) s_nsteps[threadIdx.x] += L.m;                     // history absorbed: L.m = its step count
+                if (!alive) {
+                    s_nsteps[threadIdx.x] += L.m;                             // history absorbed: L.m = its step count
+                    if (L.m >= P.max_steps) atomicAdd((unsigned long long*)&s_tally[6], 1ull);
+                }
                 if (alive) {
                     if ((unsigned)L.ix >= (unsigned)nx || (unsigned)L.iy >= (unsigned)ny || (unsigned)L.iz >= (unsigned)nz) {
                         atomicAdd((unsigned long long*)&s_tally[4],                            // left the grid
@@ -506,6 +512,7 @@ transport_kernel(const __grid_constant__ Params P)
         if (lane == 0) atomicAdd((unsigned long long*)&s_tally[c], (unsigned long long)x);
     }
     __syncthreads();
+    if (threadIdx.x == 6 && s_tally[6]) atomicAdd(&P.counters->aborted, (unsigned long long)s_tally[6]);
     if (threadIdx.x < 6) {
         unsigned long long* dst = threadIdx.x == 5 ? &P.counters->reds
                                 : threadIdx.x == 0 ? &P.counters->histories
@@ -541,6 +548,7 @@ void launch_transport(const pbs4d_grid& g, const float* rho, const DevSegment* s
     Params P;
     P.g = g; P.rho = rho; P.segs = segs; P.seg_begin = seg_begin; P.tab = static_cast<const float4*>(phys_tab_dev);
     P.n_segs = n_segs; P.hist_begin = hist_begin; P.n_hist = n_hist; P.flags = flags;
+    P.max_steps = (flags & PBS4D_TEST_STEP_CAP_64) ? 64u : (1u << 20);
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
     P.Q = (unsigned long long*)Q; P.counters = counters;

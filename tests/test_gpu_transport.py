@@ -66,6 +66,7 @@ def check_parity(g_res, o_res, label, dmax_frac=0.02):
     dose_o, Qo, sto, rho_o = o_res
     assert (rho_g == rho_o).all(), label + ": density differs"
     assert stg["histories"] == int(sto["histories"])
+    assert stg["aborted"] == 0, label + ": the step cap (hang guard) must never act on a valid plan"
     # total energy within 0.1 %
     assert abs(stg["q_deposited"] - int(sto["q_deposited"])) <= 1e-3 * int(sto["q_deposited"]), label
     assert abs(stg["q_escaped"] - int(sto["q_escaped"])) <= 1e-3 * max(int(sto["q_incident"]), 1), label
@@ -195,3 +196,22 @@ def test_batched_phases_equal_single_calls(ctx):
             assert st[k] == single[p][1][k], (p, k)
     with pytest.raises(RuntimeError):
         ctx.mc_dose_phases([phases[0], phases[0]], cfg["seed"])
+
+
+def test_step_cap_ends_every_history_and_keeps_the_energy_balance(ctx):
+    # The transport kernel is persistent: a history that could not end would hold the GPU for ever, so a history that
+    # reaches the step cap (2^20 steps; real ones need hundreds) is absorbed where it stands and counted in
+    # stats["aborted"].  No valid plan gets there, so the test switch PBS4D_TEST_STEP_CAP_64 lowers the cap to 64 steps:
+    # a 150 MeV proton in water needs ~530, hence EVERY history is stopped, after exactly 64 steps of at most one 2 mm
+    # voxel each -- and energy is still conserved, the rest being deposited on the spot.
+    cfg = synth.config1(n_hist=20_000, n=100)                           # 200 mm of water: deeper than the 157.7 mm range
+    g, dg = gpu_run(ctx, cfg, flags=binding.TEST_STEP_CAP_64)
+    dose, Q, st, _ = g[0]
+    assert st["histories"] == 20_000 and st["aborted"] == 20_000 and st["steps"] == 64 * 20_000
+    assert int(Q.sum()) == st["q_deposited"] and st["q_escaped"] == 0
+    assert abs(st["q_incident"] - st["q_deposited"]) <= 2e-5 * st["q_incident"]
+    depth = Q.sum(axis=(1, 2))
+    assert depth[64:].sum() == 0 and depth[:64].sum() > 0               # nothing beyond 64 voxels = 128 mm
+    # and the switch is a switch: the next run is the full one
+    g, _ = gpu_run(ctx, cfg)
+    assert g[0][2]["aborted"] == 0 and g[0][2]["steps"] > 400 * 20_000
